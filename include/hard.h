@@ -1,0 +1,116 @@
+/* hard.h — C-ABI boundary of hard-b200: the explicit finite-volume update of the compressible Euler
+ * equations on a uniform Cartesian mesh, the hot path of HARD (arxiv 2509.08971), on one B200.
+ *
+ * Citations: P:NNN = PAPER.md line NNN; Gn = DESIGN.md reading n; BJ = BASELINE.json north_star.
+ *
+ * What a simulation computes (eq.1-3, hydro rows, S = 0):
+ *   U = (rho, mx, my, mz, E) cell-centred conserved densities (E = e + rho v^2/2, eq.2),
+ *   ideal gas p = (gamma-1) e.  One step is Heun's method (Table 2):
+ *     U1      = U^n + dt L(U^n)
+ *     U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1))
+ *   with L(U)_i = - sum_d (F*_{i+1/2} - F*_{i-1/2})_d / Delta_d (eq.15), F* an approximate
+ *   Riemann flux of face values reconstructed from cell-centred primitives, ghost cells
+ *   filled before each stage, and dt = cfl / lambda, lambda = max over cells and active
+ *   directions of (|u_d| + c_s)/Delta_d (G6), evaluated on U^n.
+ *
+ * Layout of every state pointer: nx*ny*nz contiguous doubles, index i + nx*(j + ny*k), x fastest,
+ * interior cells only (ghost layers are internal).  A pointer may address HOST or DEVICE memory
+ * (resolved with cudaPointerGetAttributes).  The caller keeps ownership of every pointer it passes;
+ * set/get copy.  The library owns its state buffers unless hard_bind_workspace lent it memory.
+ *
+ * Errors: every int call returns HARD_OK or a negative code; nothing throws or aborts across the
+ * ABI; hard_last_error gives text.  hard_step* only enqueue work on the bound stream and return;
+ * hard_max_dt, hard_get_state and hard_get_time synchronise that stream and surface a latched
+ * HARD_ERR_NONPHYSICAL (non-finite value, rho <= 0 or p <= 0 seen by the CFL pass).
+ * A handle is not thread-safe; distinct handles are independent.  There is no CPU fallback: every
+ * call fails with HARD_ERR_CUDA when no sm_100 device is usable.
+ */
+#ifndef HARD_B200_HARD_H
+#define HARD_B200_HARD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hard_ctx hard_ctx; /* opaque, one per simulation */
+
+enum { HARD_OK = 0, HARD_ERR_ARG = -1, HARD_ERR_CUDA = -2, HARD_ERR_NOMEM = -3, HARD_ERR_NOSTATE = -4,
+       HARD_ERR_NONPHYSICAL = -5 };
+enum { HARD_BC_PERIODIC = 0, HARD_BC_OUTFLOW = 1 }; /* applied on all faces of active dimensions (G10) */
+enum { HARD_SCHEME_WENO5Z_HLL = 0,   /* the paper's scheme, P:151 (default)                       */
+       HARD_SCHEME_MUSCL_HLLC = 1 }; /* BJ fallback: MUSCL-minmod + HLLC                          */
+enum { HARD_VARIANT_FUSED = 0,       /* one kernel per RK stage (BJ "fused RK stage")             */
+       HARD_VARIANT_PERDIR = 1 };    /* one kernel per direction + axpy + CFL (BJ comparison)     */
+
+/* ---- the five calls BASELINE.json north_star names ------------------------------------------- */
+
+/* Create a simulation on an nx x ny x nz mesh.  A direction with n = 1 is inactive: no
+ * ghosts, no flux, not in the CFL maximum (G11); an active direction needs n >= 3.  gamma > 1.
+ * Spacing defaults to 1/nx, 1/ny, 1/nz.  Uses the current CUDA device.  NULL on failure (text via
+ * hard_last_error(NULL)). */
+hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc);
+
+/* Copy five conserved fields (host or device pointers, layout above) into the state, reset t = 0,
+ * fill ghosts and evaluate lambda.  Returns HARD_ERR_NONPHYSICAL if the state is not admissible. */
+int hard_set_state(hard_ctx*, const double* rho, const double* mx, const double* my, const double* mz,
+                   const double* E);
+
+/* Enqueue nsteps Heun steps, each with dt_n = cfl / lambda(U^n) evaluated on the device (no host
+ * round trip inside).  cfl > 0, nsteps >= 0. */
+int hard_step(hard_ctx*, double cfl, int nsteps);
+
+/* Synchronise and copy the five interior fields out (host or device pointers). */
+int hard_get_state(hard_ctx*, double* rho, double* mx, double* my, double* mz, double* E);
+
+/* Synchronise; *dt_out = 1 / lambda_max of the current state (so cfl * *dt_out is the next dt). */
+int hard_max_dt(hard_ctx*, double* dt_out);
+
+/* ---- extensions the configs cannot be run without ------------------------------------------- */
+
+int hard_destroy(hard_ctx*);
+
+/* Cell sizes (> 0).  Re-evaluates lambda if a state is present. */
+int hard_set_spacing(hard_ctx*, double dx, double dy, double dz);
+
+/* HARD_SCHEME_*; only before hard_set_state (ghost width 3 vs 2 changes the padded layout) and
+ * before hard_bind_workspace. */
+int hard_set_scheme(hard_ctx*, int scheme);
+
+/* HARD_VARIANT_*; may be switched at any time between steps (same state buffers). */
+int hard_set_variant(hard_ctx*, int variant);
+
+/* cudaStream_t to enqueue on (e.g. torch.cuda.current_stream().cuda_stream); default stream 0. */
+int hard_set_stream(hard_ctx*, void* cuda_stream);
+
+/* Bytes of device memory the simulation needs (state buffers + residual + scalar block). */
+size_t hard_workspace_bytes(const hard_ctx*);
+
+/* Lend the library `bytes` >= hard_workspace_bytes() of device memory aligned to 256 B (e.g. a torch
+ * tensor); the caller keeps it alive until hard_destroy.  Without this call the first
+ * hard_set_state cudaMalloc's the workspace. */
+int hard_bind_workspace(hard_ctx*, void* dev, size_t bytes);
+
+/* nsteps Heun steps with a fixed dt (end-time clamp; light-cone sub-box parity). */
+int hard_step_dt(hard_ctx*, double dt, int nsteps);
+
+/* Synchronise; simulation time and number of steps taken since hard_set_state. */
+int hard_get_time(hard_ctx*, double* t, long long* steps_done);
+
+/* Text of the last error of this handle (NULL handle: of the last failed hard_create on this thread). */
+const char* hard_last_error(const hard_ctx*);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+long long hard_launch_count(const hard_ctx*);
+
+/* Bracket the stage kernels with CUDA events on the bound stream: after hard_step returns and the
+ * stream is synchronised, *ms is the summed device time and *launches the number of stage-kernel
+ * launches (fused variant: the fused stage kernel; per-direction variant: all flux/axpy kernels)
+ * since the last call with reset != 0.  Used by bench.py for the roofline of the dominant kernel. */
+int hard_stage_time(hard_ctx*, int reset, double* ms, long long* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HARD_B200_HARD_H */

@@ -1,0 +1,478 @@
+// hard_api.cu — host side of the C-ABI declared in include/hard.h: handle, padded SoA layout in HBM,
+// tensor maps, launch sequencing of one Heun step (Table 2), set/get copies, errors.
+// No CPU fallback: every entry point fails with HARD_ERR_CUDA when CUDA is unusable.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/hard.h"
+#include "hard_kernels.cuh"
+
+using namespace hard;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct hard_ctx {
+  GridDesc g;
+  int scheme = HARD_SCHEME_WENO5Z_HLL, variant = HARD_VARIANT_FUSED;
+  cudaStream_t stream = 0;
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  bool ws_owned = false;
+  DevScalars* sc = nullptr;
+  double *U = nullptr, *U1 = nullptr, *Rres = nullptr;
+  CUtensorMap tmU, tmU1;
+  bool maps_ready = false;
+  bool have_state = false;
+  long long steps_enq = 0;          // host-side parity of the lambda ping-pong
+  long long launches = 0;
+  int Lz = 0;
+  int sm_count = 148;
+  std::string err;
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev;      // start/stop pairs around stage kernels
+  size_t ev_used = 0;
+};
+
+namespace {
+
+int fail(hard_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+int cuda_fail(hard_ctx* c, cudaError_t e, const char* where) {
+  return fail(c, HARD_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+  do {                                                            \
+    cudaError_t e__ = (call);                                     \
+    if (e__ != cudaSuccess) return cuda_fail(c, e__, #call);      \
+  } while (0)
+
+void compute_layout(hard_ctx* c) {
+  GridDesc& g = c->g;
+  g.g = (c->scheme == HARD_SCHEME_WENO5Z_HLL) ? 3 : 2;
+  for (int a = 0; a < 3; ++a) g.act[a] = g.n[a] > 1;
+  // x: interior starts at a 32-byte boundary; row pitch a multiple of 16 doubles (TMA strides must be
+  // multiples of 16 B, rows start on 128-B lines)
+  g.off[0] = g.act[0] ? 4 : 0;
+  g.off[1] = g.act[1] ? g.g : 0;
+  g.off[2] = g.act[2] ? g.g : 0;
+  g.P[0] = (int)align_up((size_t)g.off[0] + g.n[0] + (g.act[0] ? g.g : 0), 16);
+  g.P[1] = g.n[1] + 2 * g.off[1];
+  g.P[2] = g.n[2] + 2 * g.off[2];
+  g.pitch = g.P[0];
+  g.plane = g.pitch * g.P[1];
+  g.fstride = (long long)align_up((size_t)(g.plane * g.P[2]), 32);
+}
+
+size_t state_bytes(const hard_ctx* c) { return (size_t)5 * c->g.fstride * sizeof(double); }
+
+void carve(hard_ctx* c) {
+  char* p = (char*)c->ws;
+  c->sc = (DevScalars*)p;
+  p += 256;
+  const size_t sb = align_up(state_bytes(c), 256);
+  c->U = (double*)p;  p += sb;
+  c->U1 = (double*)p; p += sb;
+  c->Rres = (double*)p;
+}
+
+int make_map(hard_ctx* c, CUtensorMap* m, double* base) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !p)
+      return fail(c, HARD_ERR_CUDA, "cuTensorMapEncodeTiled entry point unavailable");
+    fn = (EncodeTiledFn)p;
+  }
+  const GridDesc& g = c->g;
+  const int T = 16, B = T + 2 * g.g;
+  cuuint64_t dims[4] = { (cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], 5 };
+  cuuint64_t strides[3] = { (cuuint64_t)g.pitch * 8, (cuuint64_t)g.plane * 8, (cuuint64_t)g.fstride * 8 };
+  cuuint32_t box[4] = { (cuuint32_t)B, (cuuint32_t)B, 1, 5 };
+  cuuint32_t es[4] = { 1, 1, 1, 1 };
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[96];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return fail(c, HARD_ERR_CUDA, buf);
+  }
+  return HARD_OK;
+}
+
+int choose_Lz(const hard_ctx* c) {
+  const GridDesc& g = c->g;
+  const long long tiles = (long long)((g.n[0] + 15) / 16) * ((g.n[1] + 15) / 16);
+  const int nz = g.n[2];
+  if (!g.act[2]) return 1;
+  const double lead = 2.0 + 0.5 * (2 * (g.g - 1) + 1);      // z-only iterations + prologue loads, in plane units
+  double best = 1e300;
+  int bestc = 1;
+  for (int ch = 1; ch <= (nz + 15) / 16; ++ch) {
+    const int lz = (nz + ch - 1) / ch;
+    const long long ctas = tiles * ((nz + lz - 1) / lz);
+    const double waves = std::ceil((double)ctas / c->sm_count);
+    const double cost = waves * (lz + lead);
+    if (cost < best * 0.999) { best = cost; bestc = ch; }
+  }
+  return (nz + bestc - 1) / bestc;
+}
+
+int ensure_ready(hard_ctx* c) {
+  if (!c->ws) {
+    const size_t need = hard_workspace_bytes(c);
+    cudaError_t e = cudaMalloc(&c->ws, need);
+    if (e != cudaSuccess) { c->ws = nullptr; return fail(c, HARD_ERR_NOMEM, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
+    c->ws_bytes = need;
+    c->ws_owned = true;
+    CK(cudaMemsetAsync(c->ws, 0, need, c->stream));
+    carve(c);
+  }
+  if (!c->maps_ready) {
+    int rc = make_map(c, &c->tmU, c->U);
+    if (rc) return rc;
+    rc = make_map(c, &c->tmU1, c->U1);
+    if (rc) return rc;
+    CK(cudaFuncSetAttribute(stage_kernel<SCHEME_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<SCHEME_A>::SMEM));
+    CK(cudaFuncSetAttribute(stage_kernel<SCHEME_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<SCHEME_B>::SMEM));
+    c->Lz = choose_Lz(c);
+    c->maps_ready = true;
+  }
+  return HARD_OK;
+}
+
+int small_grid(const hard_ctx* c, long long work) {
+  long long b = (work + 255) / 256;
+  const long long cap = (long long)c->sm_count * 8;
+  if (b > cap) b = cap;
+  if (b < 1) b = 1;
+  return (int)b;
+}
+
+int launch_ghost(hard_ctx* c, double* U, int advance, double cfl, double dt_fixed) {
+  const GridDesc& g = c->g;
+  long long work = 0;
+  if (g.act[0]) work += 2LL * g.g * g.n[1] * g.n[2];
+  if (g.act[1]) work += 2LL * g.g * g.n[0] * g.n[2];
+  if (g.act[2]) work += 2LL * g.g * g.n[0] * g.n[1];
+  ghost_fill_kernel<<<small_grid(c, work), 256, 0, c->stream>>>(U, g, c->sc, advance, (int)(c->steps_enq & 1), cfl, dt_fixed);
+  c->launches++;
+  CK(cudaGetLastError());
+  return HARD_OK;
+}
+
+int launch_cfl(hard_ctx* c, const double* U, int slot) {
+  const long long N = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2];
+  cfl_kernel<<<small_grid(c, N), 256, 0, c->stream>>>(U, c->g, c->sc, slot);
+  c->launches++;
+  CK(cudaGetLastError());
+  return HARD_OK;
+}
+
+int prof_begin(hard_ctx* c) {
+  if (!c->profiling) return HARD_OK;
+  if (c->ev_used + 2 > c->ev.size()) {
+    for (int i = 0; i < 2; ++i) {
+      cudaEvent_t e;
+      CK(cudaEventCreate(&e));
+      c->ev.push_back(e);
+    }
+  }
+  CK(cudaEventRecord(c->ev[c->ev_used], c->stream));
+  return HARD_OK;
+}
+int prof_end(hard_ctx* c) {
+  if (!c->profiling) return HARD_OK;
+  CK(cudaEventRecord(c->ev[c->ev_used + 1], c->stream));
+  c->ev_used += 2;
+  return HARD_OK;
+}
+
+int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const double* Uaux, double* Uout, int mode,
+                 int dirmask, int first, double cfl, double dt_fixed) {
+  const GridDesc& g = c->g;
+  StageArgs a;
+  a.mode = mode; a.dirmask = dirmask; a.first = first; a.cur = (int)(c->steps_enq & 1);
+  a.cfl = cfl; a.dt_fixed = dt_fixed;
+  const bool zact = g.act[2] && (dirmask & 4);
+  a.Lz = zact ? c->Lz : (g.n[2] + ((g.n[2] + 63) / 64) - 1) / ((g.n[2] + 63) / 64);   // z inactive: chunks of <= 64 planes
+  dim3 grid((g.n[0] + 15) / 16, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
+  int rc = prof_begin(c);
+  if (rc) return rc;
+  if (c->scheme == HARD_SCHEME_WENO5Z_HLL)
+    stage_kernel<SCHEME_A><<<grid, 256, StageCfg<SCHEME_A>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
+  else
+    stage_kernel<SCHEME_B><<<grid, 256, StageCfg<SCHEME_B>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
+  c->launches++;
+  CK(cudaGetLastError());
+  return prof_end(c);
+}
+
+int launch_axpy(hard_ctx* c, int stage2, double cfl, double dt_fixed) {
+  const long long N = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2];
+  int rc = prof_begin(c);
+  if (rc) return rc;
+  axpy_kernel<<<small_grid(c, N), 256, 0, c->stream>>>(c->U, c->U1, c->Rres, stage2 ? c->U : c->U1, c->g, c->sc, stage2,
+                                                        (int)(c->steps_enq & 1), cfl, dt_fixed);
+  c->launches++;
+  CK(cudaGetLastError());
+  return prof_end(c);
+}
+
+// L(Usrc) into the residual array, one launch per active direction (variant a8)
+int perdir_residual(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, double cfl, double dt_fixed) {
+  int first = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (!c->g.act[d]) continue;
+    int rc = launch_stage(c, tm, Usrc, c->Rres, c->Rres, MODE_RESID, 1 << d, first, cfl, dt_fixed);
+    if (rc) return rc;
+    first = 0;
+  }
+  return HARD_OK;
+}
+
+int do_steps(hard_ctx* c, double cfl, double dt_fixed, int nsteps) {
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
+  int rc = ensure_ready(c);
+  if (rc) return rc;
+  for (int s = 0; s < nsteps; ++s) {
+    if ((rc = launch_ghost(c, c->U, 1, cfl, dt_fixed))) return rc;
+    if (c->variant == HARD_VARIANT_FUSED) {
+      if ((rc = launch_stage(c, c->tmU, c->U, nullptr, c->U1, MODE_STAGE1, 7, 0, cfl, dt_fixed))) return rc;
+      if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
+      if ((rc = launch_stage(c, c->tmU1, c->U1, c->U, c->U, MODE_STAGE2, 7, 0, cfl, dt_fixed))) return rc;
+    } else {
+      if ((rc = perdir_residual(c, c->tmU, c->U, cfl, dt_fixed))) return rc;
+      if ((rc = launch_axpy(c, 0, cfl, dt_fixed))) return rc;
+      if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
+      if ((rc = perdir_residual(c, c->tmU1, c->U1, cfl, dt_fixed))) return rc;
+      if ((rc = launch_axpy(c, 1, cfl, dt_fixed))) return rc;
+      if ((rc = launch_cfl(c, c->U, (int)((c->steps_enq & 1) ^ 1)))) return rc;
+    }
+    c->steps_enq++;
+  }
+  return HARD_OK;
+}
+
+int sync_status(hard_ctx* c, DevScalars* host) {
+  CK(cudaMemcpyAsync(host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (host->status & 1) return fail(c, HARD_ERR_NONPHYSICAL, "non-physical state (non-finite, rho <= 0 or p <= 0)");
+  return HARD_OK;
+}
+
+int copy_field(hard_ctx* c, double* dev_field, const double* user, bool to_device) {
+  const GridDesc& g = c->g;
+  cudaMemcpy3DParms p;
+  memset(&p, 0, sizeof p);
+  cudaPitchedPtr up = make_cudaPitchedPtr((void*)user, (size_t)g.n[0] * 8, (size_t)g.n[0], (size_t)g.n[1]);
+  cudaPitchedPtr dp = make_cudaPitchedPtr((void*)dev_field, (size_t)g.pitch * 8, (size_t)g.pitch, (size_t)g.P[1]);
+  cudaPos dpos = make_cudaPos((size_t)g.off[0] * 8, (size_t)g.off[1], (size_t)g.off[2]);
+  if (to_device) { p.srcPtr = up; p.dstPtr = dp; p.dstPos = dpos; }
+  else           { p.srcPtr = dp; p.srcPos = dpos; p.dstPtr = up; }
+  p.extent = make_cudaExtent((size_t)g.n[0] * 8, (size_t)g.n[1], (size_t)g.n[2]);
+  p.kind = cudaMemcpyDefault;
+  CK(cudaMemcpy3DAsync(&p, c->stream));
+  return HARD_OK;
+}
+
+}  // namespace
+
+// ================================================================================ C ABI (include/hard.h)
+extern "C" {
+
+hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc) {
+  g_create_error.clear();
+  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != HARD_BC_PERIODIC && bc != HARD_BC_OUTFLOW)) {
+    g_create_error = "hard_create: bad argument";
+    return nullptr;
+  }
+  const int n[3] = { nx, ny, nz };
+  int nact = 0;
+  for (int a = 0; a < 3; ++a) {
+    if (n[a] > 1 && n[a] < 3) { g_create_error = "hard_create: an active direction needs n >= 3"; return nullptr; }
+    nact += n[a] > 1;
+  }
+  if (!nact) { g_create_error = "hard_create: at least one direction must have n > 1"; return nullptr; }
+  int dev = 0;
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) {
+    g_create_error = std::string("hard_create: no usable CUDA device (") + cudaGetErrorString(e) + "); there is no CPU fallback";
+    return nullptr;
+  }
+  if (prop.major < 10) {
+    g_create_error = "hard_create: kernels are built for sm_100a only";
+    return nullptr;
+  }
+  hard_ctx* c = new hard_ctx();
+  memset(&c->g, 0, sizeof c->g);
+  for (int a = 0; a < 3; ++a) { c->g.n[a] = n[a]; c->g.inv_d[a] = (double)n[a]; }
+  c->g.gamma = gamma;
+  c->g.bc = bc;
+  c->sm_count = prop.multiProcessorCount;
+  compute_layout(c);
+  return c;
+}
+
+int hard_destroy(hard_ctx* c) {
+  if (!c) return HARD_ERR_ARG;
+  cudaStreamSynchronize(c->stream);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->ws_owned && c->ws) cudaFree(c->ws);
+  delete c;
+  return HARD_OK;
+}
+
+const char* hard_last_error(const hard_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+long long hard_launch_count(const hard_ctx* c) { return c ? c->launches : -1; }
+
+int hard_set_spacing(hard_ctx* c, double dx, double dy, double dz) {
+  if (!c || !(dx > 0.0 && dy > 0.0 && dz > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_spacing: spacings must be > 0");
+  c->g.inv_d[0] = 1.0 / dx; c->g.inv_d[1] = 1.0 / dy; c->g.inv_d[2] = 1.0 / dz;
+  if (c->have_state) {
+    const int slot = (int)(c->steps_enq & 1);
+    CK(cudaMemsetAsync(&c->sc->lam_bits[slot], 0, sizeof(unsigned long long), c->stream));
+    return launch_cfl(c, c->U, slot);
+  }
+  return HARD_OK;
+}
+
+int hard_set_scheme(hard_ctx* c, int scheme) {
+  if (!c || (scheme != HARD_SCHEME_WENO5Z_HLL && scheme != HARD_SCHEME_MUSCL_HLLC))
+    return fail(c, HARD_ERR_ARG, "hard_set_scheme: unknown scheme");
+  if (c->have_state || c->ws) return fail(c, HARD_ERR_ARG, "hard_set_scheme: only before hard_set_state / hard_bind_workspace");
+  c->scheme = scheme;
+  compute_layout(c);
+  return HARD_OK;
+}
+
+int hard_set_variant(hard_ctx* c, int variant) {
+  if (!c || (variant != HARD_VARIANT_FUSED && variant != HARD_VARIANT_PERDIR))
+    return fail(c, HARD_ERR_ARG, "hard_set_variant: unknown variant");
+  c->variant = variant;
+  return HARD_OK;
+}
+
+int hard_set_stream(hard_ctx* c, void* s) {
+  if (!c) return HARD_ERR_ARG;
+  CK(cudaStreamSynchronize(c->stream));
+  c->stream = (cudaStream_t)s;
+  return HARD_OK;
+}
+
+size_t hard_workspace_bytes(const hard_ctx* c) {
+  if (!c) return 0;
+  return 256 + 3 * align_up(state_bytes(c), 256);
+}
+
+int hard_bind_workspace(hard_ctx* c, void* dev, size_t bytes) {
+  if (!c || !dev) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: null");
+  if (c->ws) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: a workspace is already bound");
+  if (bytes < hard_workspace_bytes(c) || ((uintptr_t)dev & 255)) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: too small or not 256-B aligned");
+  cudaPointerAttributes at;
+  CK(cudaPointerGetAttributes(&at, dev));
+  if (at.type != cudaMemoryTypeDevice) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: not device memory");
+  c->ws = dev;
+  c->ws_bytes = bytes;
+  c->ws_owned = false;
+  CK(cudaMemsetAsync(c->ws, 0, hard_workspace_bytes(c), c->stream));
+  carve(c);
+  return HARD_OK;
+}
+
+int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const double* my, const double* mz, const double* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return fail(c, HARD_ERR_ARG, "hard_set_state: null pointer");
+  int rc = ensure_ready(c);
+  if (rc) return rc;
+  const double* src[5] = { rho, mx, my, mz, E };
+  for (int f = 0; f < 5; ++f)
+    if ((rc = copy_field(c, c->U + f * c->g.fstride, src[f], true))) return rc;
+  CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
+  c->steps_enq = 0;
+  c->have_state = true;
+  c->err.clear();
+  if ((rc = launch_cfl(c, c->U, 0))) return rc;
+  DevScalars h;
+  return sync_status(c, &h);
+}
+
+int hard_get_state(hard_ctx* c, double* rho, double* mx, double* my, double* mz, double* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return fail(c, HARD_ERR_ARG, "hard_get_state: null pointer");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
+  double* dst[5] = { rho, mx, my, mz, E };
+  int rc;
+  for (int f = 0; f < 5; ++f)
+    if ((rc = copy_field(c, c->U + f * c->g.fstride, dst[f], false))) return rc;
+  DevScalars h;
+  return sync_status(c, &h);
+}
+
+int hard_step(hard_ctx* c, double cfl, int nsteps) {
+  if (!c || !(cfl > 0.0) || nsteps < 0) return fail(c, HARD_ERR_ARG, "hard_step: cfl > 0 and nsteps >= 0 required");
+  return do_steps(c, cfl, 0.0, nsteps);
+}
+
+int hard_step_dt(hard_ctx* c, double dt, int nsteps) {
+  if (!c || !(dt > 0.0) || nsteps < 0) return fail(c, HARD_ERR_ARG, "hard_step_dt: dt > 0 and nsteps >= 0 required");
+  return do_steps(c, 1.0, dt, nsteps);
+}
+
+int hard_max_dt(hard_ctx* c, double* dt_out) {
+  if (!c || !dt_out) return fail(c, HARD_ERR_ARG, "hard_max_dt: null");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
+  DevScalars h;
+  int rc = sync_status(c, &h);
+  double lam;
+  memcpy(&lam, &h.lam_bits[c->steps_enq & 1], sizeof lam);
+  *dt_out = 1.0 / lam;
+  return rc;
+}
+
+int hard_get_time(hard_ctx* c, double* t, long long* steps_done) {
+  if (!c) return HARD_ERR_ARG;
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
+  DevScalars h;
+  int rc = sync_status(c, &h);
+  if (t) *t = h.t;
+  if (steps_done) *steps_done = h.steps;
+  return rc;
+}
+
+int hard_stage_time(hard_ctx* c, int reset, double* ms, long long* launches) {
+  if (!c) return HARD_ERR_ARG;
+  CK(cudaStreamSynchronize(c->stream));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    float f = 0.f;
+    CK(cudaEventElapsedTime(&f, c->ev[i], c->ev[i + 1]));
+    tot += f;
+  }
+  if (ms) *ms = tot;
+  if (launches) *launches = (long long)(c->ev_used / 2);
+  if (reset) { c->ev_used = 0; c->profiling = true; }
+  return HARD_OK;
+}
+
+}  // extern "C"

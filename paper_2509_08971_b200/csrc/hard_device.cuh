@@ -1,0 +1,144 @@
+// hard_device.cuh — device arithmetic of the hot path (sm_100a): conserved->primitive with the
+// ideal-gas EOS, limited face reconstruction, approximate Riemann fluxes.  Written from PAPER.md
+// (eq.2-3) and the DESIGN.md readings; shares nothing with oracle/.
+//
+// Precision: everything is fp64.  Unlike the oracle (correctly rounded ops in a fixed order, no FMA
+// contraction) this code lets nvcc contract to DFMA and regroups sums; DESIGN.md "Tolerance"
+// derives why that stays inside 1e-12 (one step) / 1e-9 (100 steps).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace hard {
+
+constexpr int SCHEME_A = 0;   // WENO5-Z + HLL
+constexpr int SCHEME_B = 1;   // MUSCL-minmod + HLLC (BASELINE.json north_star fallback)
+
+template <int S> struct SchemeTraits;
+template <> struct SchemeTraits<SCHEME_A> { static constexpr int G = 3, R = 2; };
+template <> struct SchemeTraits<SCHEME_B> { static constexpr int G = 2, R = 1; };
+
+// a2 (eq.2): (rho, mx, my, mz, E) -> (rho, u, v, w, p).
+__device__ __forceinline__ void cons_to_prim(const double U[5], double gm1, double W[5]) {
+  const double inv = 1.0 / U[0];
+  W[0] = U[0];
+  W[1] = U[1] * inv;
+  W[2] = U[2] * inv;
+  W[3] = U[3] * inv;
+  W[4] = gm1 * (U[4] - 0.5 * (U[1] * W[1] + U[2] * W[2] + U[3] * W[3]));
+}
+
+// a3, scheme A (Borges et al. [18]; G1: eps = 1e-40, power 1, d = (1/10, 6/10, 3/10)).
+// Both face values of cell i from q[i-2..i+2] = (a,b,c,d,e): plus at i+1/2, minus at i-1/2.  The
+// minus value is the same function on the mirrored stencil, so the smoothness indicators and
+// tau/(beta+eps) ratios are shared: beta0' = beta2, beta1' = beta1, beta2' = beta0.
+__device__ __forceinline__ void wenoz_pair(double a, double b, double c, double d, double e, double& plus,
+                                           double& minus) {
+  const double eps = 1e-40;
+  const double s0 = (a - 2.0 * b) + c, t0 = (a - 4.0 * b) + 3.0 * c;
+  const double s1 = (b - 2.0 * c) + d, t1 = b - d;
+  const double s2 = (c - 2.0 * d) + e, t2 = (3.0 * c - 4.0 * d) + e;
+  const double b0 = (13.0 / 12.0) * (s0 * s0) + 0.25 * (t0 * t0);
+  const double b1 = (13.0 / 12.0) * (s1 * s1) + 0.25 * (t1 * t1);
+  const double b2 = (13.0 / 12.0) * (s2 * s2) + 0.25 * (t2 * t2);
+  const double tau = fabs(b0 - b2);
+  // r_k = tau / (beta_k + eps) with ONE reciprocal: 1/(B0 B1 B2).  beta <= ~1e17 for admissible
+  // data of the configs, eps^3 = 1e-120: no overflow / underflow in fp64.
+  const double B0 = b0 + eps, B1 = b1 + eps, B2 = b2 + eps;
+  const double B01 = B0 * B1;
+  const double ti = tau * (1.0 / (B01 * B2));
+  const double r0 = ti * (B1 * B2), r1 = ti * (B0 * B2), r2 = ti * B01;
+  const double q0 = (1.0 / 6.0) * ((2.0 * a - 7.0 * b) + 11.0 * c);
+  const double q1 = (1.0 / 6.0) * ((5.0 * c - b) + 2.0 * d);
+  const double q2 = (1.0 / 6.0) * ((2.0 * c + 5.0 * d) - e);
+  const double p0 = (1.0 / 6.0) * ((2.0 * e - 7.0 * d) + 11.0 * c);
+  const double p1 = (1.0 / 6.0) * ((5.0 * c - d) + 2.0 * b);
+  const double p2 = (1.0 / 6.0) * ((2.0 * c + 5.0 * b) - a);
+  const double a0 = fma(0.1, r0, 0.1), a1 = fma(0.6, r1, 0.6), a2 = fma(0.3, r2, 0.3);   // plus
+  const double m0 = fma(0.1, r2, 0.1), m1 = a1, m2 = fma(0.3, r0, 0.3);                  // minus
+  const double sp = (a0 + a1) + a2, sm = (m0 + m1) + m2;
+  const double np = (a0 * q0 + a1 * q1) + a2 * q2;
+  const double nm = (m0 * p0 + m1 * p1) + m2 * p2;
+  const double inv = 1.0 / (sp * sm);                     // sp, sm in [1, ~1e57]: safe
+  plus = np * (inv * sm);
+  minus = nm * (inv * sp);
+}
+
+// a3, scheme B: MUSCL with the minmod limiter, sign tests (no product).
+__device__ __forceinline__ void minmod_pair(double b, double c, double d, double& plus, double& minus) {
+  const double x = c - b, y = d - c;
+  double s = 0.0;
+  if (x > 0.0 && y > 0.0) s = fmin(x, y);
+  else if (x < 0.0 && y < 0.0) s = fmax(x, y);
+  plus = fma(0.5, s, c);
+  minus = fma(-0.5, s, c);
+}
+
+// a4 (G2 Davis bounds; G5 inclusive tie-breaks).  WL/WR = (rho, un, ut1, ut2, p) already
+// rotated so that component 1 is the face normal.  F in the same rotated (rho, n, t1, t2, E) order.
+template <int S>
+__device__ __forceinline__ void riemann_flux(const double WL[5], const double WR[5], double gamma, double inv_gm1,
+                                             double F[5]) {
+  const double cL = sqrt(gamma * WL[4] / WL[0]);
+  const double cR = sqrt(gamma * WR[4] / WR[0]);
+  const double SL = fmin(WL[1] - cL, WR[1] - cR);
+  const double SR = fmax(WL[1] + cL, WR[1] + cR);
+  const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));
+  const double ER = WR[4] * inv_gm1 + 0.5 * WR[0] * (WR[1] * WR[1] + (WR[2] * WR[2] + WR[3] * WR[3]));
+  const double UL[5] = { WL[0], WL[0] * WL[1], WL[0] * WL[2], WL[0] * WL[3], EL };
+  const double UR[5] = { WR[0], WR[0] * WR[1], WR[0] * WR[2], WR[0] * WR[3], ER };
+  const double FL[5] = { UL[1], UL[1] * WL[1] + WL[4], UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
+  const double FR[5] = { UR[1], UR[1] * WR[1] + WR[4], UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
+  if (SL >= 0.0) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) F[m] = FL[m];
+    return;
+  }
+  if (SR <= 0.0) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) F[m] = FR[m];
+    return;
+  }
+  if (S == SCHEME_A) {                                   // HLL
+    const double inv = 1.0 / (SR - SL);
+    const double ss = SL * SR;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) F[m] = ((SR * FL[m] - SL * FR[m]) + ss * (UR[m] - UL[m])) * inv;
+  } else {                                               // HLLC, averaged-pressure form (G5)
+    const double A = WL[0] * (SL - WL[1]);
+    const double B = WR[0] * (SR - WR[1]);
+    const double Ss = ((WR[4] - WL[4]) + (A * WL[1] - B * WR[1])) / (A - B);
+    const double pbar = 0.5 * ((WL[4] + WR[4]) + (A * (Ss - WL[1]) + B * (Ss - WR[1])));
+    if (Ss == 0.0) {
+      F[0] = 0.0; F[1] = pbar; F[2] = 0.0; F[3] = 0.0; F[4] = 0.0;
+      return;
+    }
+    const bool left = Ss > 0.0;
+    const double SK = left ? SL : SR;
+    const double inv = 1.0 / (SK - Ss);
+    const double sp = SK * pbar;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      const double UK = left ? UL[m] : UR[m];
+      const double FK = left ? FL[m] : FR[m];
+      const double D = (m == 1) ? 1.0 : (m == 4) ? Ss : 0.0;
+      F[m] = (Ss * (SK * UK - FK) + sp * D) * inv;
+    }
+  }
+}
+
+// a7 building block for the fused epilogue: local max wavespeed of one conserved state; returns a
+// negative value if the state is not admissible (non-finite, rho <= 0 or p <= 0).
+__device__ __forceinline__ double cell_lambda(const double U[5], double gamma, double gm1, const double inv_d[3],
+                                              const bool act[3]) {
+  double W[5];
+  cons_to_prim(U, gm1, W);
+  if (!(W[0] > 0.0 && W[4] > 0.0) || !(W[4] < 1.0e300)) return -1.0;
+  const double c = sqrt(gamma * W[4] / W[0]);
+  double lam = 0.0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+    if (act[a]) lam = fmax(lam, (fabs(W[1 + a]) + c) * inv_d[a]);
+  return lam;
+}
+
+}  // namespace hard

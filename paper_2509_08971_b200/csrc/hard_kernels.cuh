@@ -1,0 +1,448 @@
+// hard_kernels.cuh — CUDA kernels of the hot path for sm_100a:
+//   ghost_fill_kernel   a1  ghost-cell fill, all faces of active directions, one launch
+//   stage_kernel<S>     a2..a6 (+a7 fused in stage 2): TMA-staged x-y tile marched along z
+//   cfl_kernel          a7  standalone max-wavespeed reduction (set_state, per-direction variant)
+//   axpy_kernel         a6  RK combination of the per-direction variant (a8)
+// The stage kernel also serves the per-direction comparison variant (a8): dirmask selects one
+// direction and MODE_RESID read-modify-writes a residual array instead of applying the RK update.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "hard_device.cuh"
+
+namespace hard {
+
+struct GridDesc {
+  int n[3];                 // interior cells
+  int off[3];               // padded coordinate of interior cell 0 (>= ghost width; 0 if inactive)
+  int act[3];               // n > 1
+  int P[3];                 // padded extents: P[0] = row pitch (doubles), P[1], P[2]
+  long long pitch, plane, fstride;   // doubles: row, z-plane, field
+  double inv_d[3];
+  double gamma;
+  int bc;                   // 0 periodic, 1 outflow
+  int g;                    // ghost width of the scheme
+};
+
+// Device-resident scalars: nothing returns to the host inside hard_step.
+struct DevScalars {
+  unsigned long long lam_bits[2];   // ping-pong max wavespeed (bit pattern of a non-negative double)
+  double t, dt_last;
+  long long steps;
+  int status;                       // bit 0: non-physical state seen
+  int pad;
+};
+
+enum { MODE_STAGE1 = 0, MODE_STAGE2 = 1, MODE_RESID = 2 };
+
+struct StageArgs {
+  int mode;
+  int dirmask;      // bit d: take direction d's fluxes (fused: 7)
+  int first;        // MODE_RESID: overwrite instead of accumulate
+  int Lz;           // planes per z-chunk
+  int cur;          // lam_bits[cur] is lambda(U^n); stage 2 accumulates into lam_bits[cur^1]
+  double cfl, dt_fixed;   // dt = dt_fixed > 0 ? dt_fixed : cfl / lambda
+};
+
+__device__ __forceinline__ double step_dt(const DevScalars* sc, int cur, double cfl, double dt_fixed) {
+  if (dt_fixed > 0.0) return dt_fixed;
+  return __ddiv_rn(cfl, __longlong_as_double((long long)sc->lam_bits[cur]));
+}
+
+__device__ __forceinline__ long long cell_addr(const GridDesc& g, int i, int j, int k) {
+  return (long long)(i + g.off[0]) + g.pitch * (long long)(j + g.off[1]) + g.plane * (long long)(k + g.off[2]);
+}
+
+// ------------------------------------------------------------------------------------------- a1
+// One thread per ghost cell (all five fields).  Index space: [x faces | y faces | z faces]; x-face
+// threads are laid out layer-fastest, y/z-face threads x-fastest (coalesced).  Thread 0 also
+// advances the device clock when `advance` (first fill of a step) and clears the lambda slot the
+// step will reduce into.
+__global__ void ghost_fill_kernel(double* __restrict__ U, GridDesc g, DevScalars* sc, int advance, int cur,
+                                  double cfl, double dt_fixed) {
+  if (advance && blockIdx.x == 0 && threadIdx.x == 0) {
+    const double dt = step_dt(sc, cur, cfl, dt_fixed);
+    sc->lam_bits[cur ^ 1] = 0ull;
+    sc->t += dt;
+    sc->dt_last = dt;
+    sc->steps += 1;
+  }
+  const int G = g.g;
+  const long long nx = g.n[0], ny = g.n[1], nz = g.n[2];
+  const long long cx = g.act[0] ? 2LL * G * ny * nz : 0;
+  const long long cy = g.act[1] ? 2LL * G * nx * nz : 0;
+  const long long cz = g.act[2] ? 2LL * G * nx * ny : 0;
+  const long long total = cx + cy + cz;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    int d, m, c[3];
+    if (idx < cx) {
+      d = 0; m = (int)(idx % (2 * G));
+      long long r = idx / (2 * G);
+      c[1] = (int)(r % ny); c[2] = (int)(r / ny);
+    } else if (idx < cx + cy) {
+      long long r = idx - cx;
+      d = 1; c[0] = (int)(r % nx); r /= nx;
+      m = (int)(r % (2 * G)); c[2] = (int)(r / (2 * G));
+    } else {
+      long long r = idx - cx - cy;
+      d = 2; c[0] = (int)(r % nx); r /= nx;
+      c[1] = (int)(r % ny); m = (int)(r / ny);
+    }
+    const int n = g.n[d];
+    int dst, src;
+    if (m < G) {                                    // low side, layer m+1
+      dst = -(m + 1);
+      src = (g.bc == 0) ? n - (m + 1) : 0;
+    } else {                                        // high side, layer m-G+1
+      const int l = m - G;
+      dst = n + l;
+      src = (g.bc == 0) ? l : n - 1;
+    }
+    c[d] = dst; const long long pd = cell_addr(g, c[0], c[1], c[2]);
+    c[d] = src; const long long ps = cell_addr(g, c[0], c[1], c[2]);
+#pragma unroll
+    for (int f = 0; f < 5; ++f) U[f * g.fstride + pd] = U[f * g.fstride + ps];
+  }
+}
+
+// ------------------------------------------------------------------------------------------- a7
+__device__ __forceinline__ double sum3_sorted(double a, double b, double c) {
+  // magnitude-ordered three-term sum (G8) so that lambda after set_state is bit-equal to
+  // the definition evaluated in any axis order.
+  double x1 = a, x2 = b, x3 = c, t;
+  if (fabs(x1) > fabs(x2)) { t = x1; x1 = x2; x2 = t; }
+  if (fabs(x2) > fabs(x3)) { t = x2; x2 = x3; x3 = t; }
+  if (fabs(x1) > fabs(x2)) { t = x1; x1 = x2; x2 = t; }
+  if (x2 == -x3) return x1;
+  return __dadd_rn(__dadd_rn(x1, x2), x3);
+}
+
+__device__ __forceinline__ void block_max_to_slot(double lam, int bad, DevScalars* sc, int slot, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lam = fmax(lam, __shfl_xor_sync(0xffffffffu, lam, o));
+    bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+  }
+  const int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  if ((threadIdx.x & 31) == 0) { red[w] = lam; red[32 + w] = (double)bad; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int i = 1; i < nw; ++i) { lam = fmax(lam, red[i]); bad |= (red[32 + i] != 0.0); }
+    // lambda >= 0: the IEEE bit pattern is order-preserving as an unsigned integer; max is exact
+    // and order-independent, so dt is reproducible run to run.
+    atomicMax(&sc->lam_bits[slot], (unsigned long long)__double_as_longlong(lam));
+    if (bad) atomicOr(&sc->status, 1);
+  }
+}
+
+// Standalone CFL pass, correctly rounded operations in the order of the definition (G6, G9).
+__global__ void cfl_kernel(const double* __restrict__ U, GridDesc g, DevScalars* sc, int slot) {
+  __shared__ double red[64];
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  double lam = 0.0;
+  int bad = 0;
+  const double gm1 = __dadd_rn(g.gamma, -1.0);
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < N;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % g.n[0]);
+    const long long r = idx / g.n[0];
+    const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+    const long long p = cell_addr(g, i, j, k);
+    const double rho = U[p], mx = U[g.fstride + p], my = U[2 * g.fstride + p], mz = U[3 * g.fstride + p],
+                 E = U[4 * g.fstride + p];
+    const double v[3] = { __ddiv_rn(mx, rho), __ddiv_rn(my, rho), __ddiv_rn(mz, rho) };
+    const double ke2 = sum3_sorted(__dmul_rn(mx, v[0]), __dmul_rn(my, v[1]), __dmul_rn(mz, v[2]));
+    const double pr = __dmul_rn(gm1, __dadd_rn(E, -__dmul_rn(0.5, ke2)));
+    if (!(rho > 0.0 && pr > 0.0) || !(pr < 1.0e300) || !(rho < 1.0e300)) { bad = 1; continue; }
+    const double c = __dsqrt_rn(__ddiv_rn(__dmul_rn(g.gamma, pr), rho));
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      if (g.act[a]) lam = fmax(lam, __dmul_rn(__dadd_rn(fabs(v[a]), c), g.inv_d[a]));
+  }
+  block_max_to_slot(lam, bad, sc, slot, red);
+}
+
+// ------------------------------------------------------------------------------------------- a6 (per-direction variant)
+// stage 1: U1 = U + dt R;   stage 2: U = 1/2 U + 1/2 (U1 + dt R).   Interior cells only.
+__global__ void axpy_kernel(const double* __restrict__ Un, const double* __restrict__ U1, const double* __restrict__ R,
+                            double* __restrict__ out, GridDesc g, const DevScalars* sc, int stage2, int cur,
+                            double cfl, double dt_fixed) {
+  const double dt = step_dt(sc, cur, cfl, dt_fixed);
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < N;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % g.n[0]);
+    const long long r = idx / g.n[0];
+    const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+    const long long p = cell_addr(g, i, j, k);
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      const long long q = f * g.fstride + p;
+      if (!stage2) out[q] = fma(dt, R[q], Un[q]);
+      else out[q] = 0.5 * Un[q] + 0.5 * fma(dt, R[q], U1[q]);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------- TMA / mbarrier PTX
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HARD_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HARD_DONE;\n"
+      "bra HARD_WAIT;\n"
+      "HARD_DONE:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// 4-D tiled TMA load (x, y, z, field) of one x-y box of one z-plane, all five fields.
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int cx, int cy, int cz,
+                                            int cf) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+      ::"r"(dst), "l"((unsigned long long)map), "r"(cx), "r"(cy), "r"(cz), "r"(cf), "r"(bar) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------- a2..a7 fused stage
+template <int S>
+struct StageCfg {
+  static constexpr int G = SchemeTraits<S>::G, R = SchemeTraits<S>::R;
+  static constexpr int T = 16;                         // x-y tile edge (cells); 256 threads, one per cell
+  static constexpr int NT = T * T;
+  static constexpr int BX = T + 2 * G, BY = T + 2 * G; // TMA box
+  static constexpr int VS = BX * BY;                   // doubles per field per plane slot
+  static constexpr int SLOT = (5 * VS + 15) / 16 * 16; // slot stride, multiple of 128 B
+  static constexpr int NS = 2 * R + 2;                 // ring: z window 2R+1 plus one plane in flight
+  static constexpr int NXI = (T + 2) * T;              // x (or y) reconstruction items per plane
+  static constexpr int XB = NT, YB = NT + NXI;         // item bases: [z | x | y]
+  static constexpr int NIT = NT + 2 * NXI;
+  static constexpr uint32_t BOX_BYTES = 5u * VS * 8u;
+  static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * 5 * NIT * 8 + NS * 8 + 64 * 8 + 128;
+};
+
+// Reconstruct both face values of all five primitives of one item (cell + direction).
+// o[s] = ring offset (doubles) of field 0 at stencil position s - R.
+template <int S>
+__device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double pl[5], double mi[5]) {
+  constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S>::VS;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    if (S == SCHEME_A) {
+      wenoz_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], ring[o[3] + v * VS],
+                 ring[o[4] + v * VS], pl[v], mi[v]);
+    } else {
+      minmod_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], pl[v], mi[v]);
+    }
+  }
+  if (S == SCHEME_A) {                                   // G4 positivity fallback: piecewise constant
+    if (pl[0] <= 0.0 || pl[4] <= 0.0 || mi[0] <= 0.0 || mi[4] <= 0.0) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) pl[v] = mi[v] = ring[o[R] + v * VS];
+    }
+  }
+}
+
+template <int S>
+__global__ void __launch_bounds__(256, 1)
+stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict__ Usrc, const double* Uaux,
+             double* Uout, GridDesc g, DevScalars* sc, StageArgs a) {
+  using C = StageCfg<S>;
+  constexpr int G = C::G, R = C::R, T = C::T, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS, NIT = C::NIT,
+                XB = C::XB, YB = C::YB;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* ring = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  double* RP = ring + NS * SLOT;       // plus values; overwritten in place by the face fluxes
+  double* RM = RP + 5 * NIT;           // minus values
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(RM + 5 * NIT);
+  double* red = reinterpret_cast<double*>(bars + NS);
+
+  const int tid = threadIdx.x, tx = tid & (T - 1), ty = tid / T;
+  const int i0 = blockIdx.x * T, j0 = blockIdx.y * T, k0 = blockIdx.z * a.Lz;
+  const int kend = min(g.n[2], k0 + a.Lz);
+  const bool ax = g.act[0] && (a.dirmask & 1), ay = g.act[1] && (a.dirmask & 2), az = g.act[2] && (a.dirmask & 4);
+  const int rows = min(T, g.n[1] - j0), cols = min(T, g.n[0] - i0);
+  const bool mine = tx < cols && ty < rows;
+  const double gamma = g.gamma, gm1 = gamma - 1.0, inv_gm1 = 1.0 / gm1;
+  const double dt = step_dt(sc, a.cur, a.cfl, a.dt_fixed);
+
+  // z window of iteration kk: planes [kk + ld - rz, kk + ld + rz]; with z active the z stencil runs
+  // one plane ahead so that both z faces of plane kk are known when its x/y fluxes are.
+  const int ld = az ? 1 : 0, rz = az ? R : 0;
+  const int kfirst = az ? k0 - 2 : k0;
+  const int zb = kfirst + ld - rz;                     // first plane ever loaded; ring slot = (z - zb) % NS
+  const int cx = g.off[0] + i0 - G, cy = g.off[1] + j0 - G;
+
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) mbar_init(smem_u32(&bars[s]), 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  auto issue = [&](int z) {                            // one thread
+    const int q = z - zb, slot = q % NS;
+    const uint32_t bar = smem_u32(&bars[slot]);
+    mbar_expect_tx(bar, C::BOX_BYTES);
+    tma_load_4d(smem_u32(ring + slot * SLOT), &tmap, bar, cx, cy, g.off[2] + z, 0);
+  };
+  auto wait_convert = [&](int z) {                     // all threads: wait, conserved -> primitive in place (a2)
+    const int q = z - zb, slot = q % NS;
+    mbar_wait(smem_u32(&bars[slot]), (uint32_t)((q / NS) & 1));
+    double* sl = ring + slot * SLOT;
+    for (int c = tid; c < VS; c += C::NT) {
+      double U[5], W[5];
+#pragma unroll
+      for (int v = 0; v < 5; ++v) U[v] = sl[v * VS + c];
+      cons_to_prim(U, gm1, W);
+#pragma unroll
+      for (int v = 1; v < 5; ++v) sl[v * VS + c] = W[v];
+    }
+  };
+
+  if (tid == 0)
+    for (int z = zb; z <= zb + 2 * rz; ++z) issue(z);
+  for (int z = zb; z <= zb + 2 * rz; ++z) wait_convert(z);
+  __syncthreads();
+
+  double zplus[5] = { 0, 0, 0, 0, 0 }, Fzold[5] = { 0, 0, 0, 0, 0 }, Fznew[5] = { 0, 0, 0, 0, 0 };
+  double lam_loc = 0.0;
+  int bad = 0;
+  const bool act3[3] = { g.act[0] != 0, g.act[1] != 0, g.act[2] != 0 };
+
+  for (int kk = kfirst; kk < kend; ++kk) {
+    const bool doxy = kk >= k0;
+    const int znext = kk + 1 + ld + rz;
+    const bool more = kk + 1 < kend;
+    if (more && tid == 0) {                            // prefetch the plane the next iteration adds
+      fence_proxy_async();                             // its slot was last touched by generic-proxy accesses
+      issue(znext);
+    }
+    // own-cell conserved values for the RK combination: issued now, consumed after the flux phases
+    double uc[5] = { 0, 0, 0, 0, 0 }, ua[5] = { 0, 0, 0, 0, 0 };
+    long long pc = 0;
+    if (doxy && mine) {
+      pc = cell_addr(g, i0 + tx, j0 + ty, kk);
+      if (a.mode != MODE_RESID) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) uc[v] = Usrc[v * g.fstride + pc];
+      }
+      if (a.mode == MODE_STAGE2 || (a.mode == MODE_RESID && !a.first)) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) ua[v] = Uaux[v * g.fstride + pc];
+      }
+    }
+
+    // ---- a3: reconstruction items [z: own cell of plane kk+1 | x: (T+2) x rows | y: T x (rows+2)]
+    const int slot_c = ((kk - zb) % NS) * SLOT;        // plane kk (x/y stencils)
+    const int L0 = az ? C::NT : 0;
+    const int L1 = L0 + ((doxy && ax) ? (T + 2) * rows : 0);
+    const int L2 = L1 + ((doxy && ay) ? T * (rows + 2) : 0);
+    for (int it = tid; it < L2; it += C::NT) {
+      int o[2 * R + 1], st;
+      if (it < L0) {
+        st = it;
+        const int cell = (ty + G) * BX + (tx + G);
+#pragma unroll
+        for (int s = -R; s <= R; ++s) o[s + R] = ((kk + 1 + s - zb) % NS) * SLOT + cell;
+      } else if (it < L1) {
+        const int j = it - L0, row = j / (T + 2), c = j - row * (T + 2);
+        st = XB + j;
+        const int cell = slot_c + (row + G) * BX + (c - 1 + G);
+#pragma unroll
+        for (int s = -R; s <= R; ++s) o[s + R] = cell + s;
+      } else {
+        const int j = it - L1, c = j / T, ix = j - c * T;
+        st = YB + j;
+        const int cell = slot_c + (c - 1 + G) * BX + (ix + G);
+#pragma unroll
+        for (int s = -R; s <= R; ++s) o[s + R] = cell + s * BX;
+      }
+      double pl[5], mi[5];
+      recon_item<S>(ring, o, pl, mi);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) { RP[v * NIT + st] = pl[v]; RM[v * NIT + st] = mi[v]; }
+    }
+    __syncthreads();
+
+    // ---- a4: each face flux once.  z face kk+1/2 in registers (left state carried from the
+    // previous plane); x / y faces from the item arrays, flux written over the left item's plus slot.
+    if (az) {
+      if (kk >= k0 - 1) {
+        const double WL[5] = { zplus[0], zplus[3], zplus[1], zplus[2], zplus[4] };          // (n,t1,t2) = (w,u,v)
+        const double WR[5] = { RM[0 * NIT + tid], RM[3 * NIT + tid], RM[1 * NIT + tid], RM[2 * NIT + tid],
+                               RM[4 * NIT + tid] };
+        double F[5];
+        riemann_flux<S>(WL, WR, gamma, inv_gm1, F);
+        Fznew[0] = F[0]; Fznew[3] = F[1]; Fznew[1] = F[2]; Fznew[2] = F[3]; Fznew[4] = F[4];
+      }
+#pragma unroll
+      for (int v = 0; v < 5; ++v) zplus[v] = RP[v * NIT + tid];
+    }
+    if (doxy) {
+      const int nxf = ax ? (T + 1) * rows : 0;
+      const int nyf = ay ? T * (rows + 1) : 0;
+      for (int it = tid; it < nxf + nyf; it += C::NT) {
+        int Li, Ri, d;
+        if (it < nxf) {
+          const int row = it / (T + 1), c = it - row * (T + 1);
+          Li = XB + row * (T + 2) + c; Ri = Li + 1; d = 0;
+        } else {
+          const int j = it - nxf;
+          Li = YB + j; Ri = Li + T; d = 1;
+        }
+        const int vn = 1 + d, vt1 = 1 + (d + 1) % 3, vt2 = 1 + (d + 2) % 3;
+        const double WL[5] = { RP[Li], RP[vn * NIT + Li], RP[vt1 * NIT + Li], RP[vt2 * NIT + Li], RP[4 * NIT + Li] };
+        const double WR[5] = { RM[Ri], RM[vn * NIT + Ri], RM[vt1 * NIT + Ri], RM[vt2 * NIT + Ri], RM[4 * NIT + Ri] };
+        double F[5];
+        riemann_flux<S>(WL, WR, gamma, inv_gm1, F);
+        RP[Li] = F[0]; RP[vn * NIT + Li] = F[1]; RP[vt1 * NIT + Li] = F[2]; RP[vt2 * NIT + Li] = F[3];
+        RP[4 * NIT + Li] = F[4];
+      }
+    }
+    __syncthreads();
+
+    // ---- a5 + a6 (+ a7): divergence in registers, RK combination, store
+    if (doxy && mine) {
+      double out[5];
+      const int xi = XB + ty * (T + 2) + tx, yi = YB + ty * T + tx;
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        double L = 0.0;
+        if (ax) L -= (RP[v * NIT + xi + 1] - RP[v * NIT + xi]) * g.inv_d[0];
+        if (ay) L -= (RP[v * NIT + yi + T] - RP[v * NIT + yi]) * g.inv_d[1];
+        if (az) L -= (Fznew[v] - Fzold[v]) * g.inv_d[2];
+        if (a.mode == MODE_STAGE1) out[v] = fma(dt, L, uc[v]);
+        else if (a.mode == MODE_STAGE2) out[v] = 0.5 * ua[v] + 0.5 * fma(dt, L, uc[v]);
+        else out[v] = a.first ? L : ua[v] + L;
+        Uout[v * g.fstride + pc] = out[v];
+      }
+      if (a.mode == MODE_STAGE2) {
+        const double l = cell_lambda(out, gamma, gm1, g.inv_d, act3);
+        if (l < 0.0) bad = 1; else lam_loc = fmax(lam_loc, l);
+      }
+    }
+    if (az) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) Fzold[v] = Fznew[v];
+    }
+    if (more) wait_convert(znext);
+    __syncthreads();
+  }
+  if (a.mode == MODE_STAGE2) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
+}
+
+}  // namespace hard
