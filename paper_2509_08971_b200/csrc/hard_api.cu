@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -45,6 +46,7 @@ struct hard_ctx {
   int sm_count = 148;
   std::string err;
   bool profiling = false;
+  bool debug_sync = false;            // HARD_DEBUG_SYNC=1: synchronise and check after every launch
   std::vector<cudaEvent_t> ev;      // start/stop pairs around stage kernels
   size_t ev_used = 0;
 };
@@ -58,19 +60,31 @@ int fail(hard_ctx* c, int code, const std::string& msg) {
 int cuda_fail(hard_ctx* c, cudaError_t e, const char* where) {
   return fail(c, HARD_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
 }
+int after_launch(hard_ctx* c, const char* name);
 #define CK(call)                                                  \
   do {                                                            \
     cudaError_t e__ = (call);                                     \
     if (e__ != cudaSuccess) return cuda_fail(c, e__, #call);      \
   } while (0)
 
+int after_launch(hard_ctx* c, const char* name) {
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess && c->debug_sync) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, e, name);
+  return HARD_OK;
+}
+
 void compute_layout(hard_ctx* c) {
   GridDesc& g = c->g;
   g.g = (c->scheme == HARD_SCHEME_WENO5Z_HLL) ? 3 : 2;
   for (int a = 0; a < 3; ++a) g.act[a] = g.n[a] > 1;
-  // x: interior starts at a 32-byte boundary; row pitch a multiple of 16 doubles (TMA strides must be
-  // multiples of 16 B, rows start on 128-B lines)
-  g.off[0] = g.act[0] ? 4 : 0;
+  // x: ghost width g on the left, so that a tile's TMA box (which starts g cells left of the tile)
+  // starts at padded x-coordinate i0, a multiple of 16 doubles: the box start must be 16-byte
+  // aligned (measured: an odd fp64 start coordinate raises "illegal instruction" on sm_100a) and
+  // every box row then starts on a 128-B line.  Row pitch: a multiple of 16 doubles (TMA strides
+  // must be multiples of 16 B).
+  g.off[0] = g.g;   // also when x is inactive (the columns stay zero and are never read by a valid cell)
   g.off[1] = g.act[1] ? g.g : 0;
   g.off[2] = g.act[2] ? g.g : 0;
   g.P[0] = (int)align_up((size_t)g.off[0] + g.n[0] + (g.act[0] ? g.g : 0), 16);
@@ -175,17 +189,13 @@ int launch_ghost(hard_ctx* c, double* U, int advance, double cfl, double dt_fixe
   if (g.act[1]) work += 2LL * g.g * g.n[0] * g.n[2];
   if (g.act[2]) work += 2LL * g.g * g.n[0] * g.n[1];
   ghost_fill_kernel<<<small_grid(c, work), 256, 0, c->stream>>>(U, g, c->sc, advance, (int)(c->steps_enq & 1), cfl, dt_fixed);
-  c->launches++;
-  CK(cudaGetLastError());
-  return HARD_OK;
+  return after_launch(c, "ghost_fill_kernel");
 }
 
 int launch_cfl(hard_ctx* c, const double* U, int slot) {
   const long long N = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2];
   cfl_kernel<<<small_grid(c, N), 256, 0, c->stream>>>(U, c->g, c->sc, slot);
-  c->launches++;
-  CK(cudaGetLastError());
-  return HARD_OK;
+  return after_launch(c, "cfl_kernel");
 }
 
 int prof_begin(hard_ctx* c) {
@@ -222,8 +232,7 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
     stage_kernel<SCHEME_A><<<grid, 256, StageCfg<SCHEME_A>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
   else
     stage_kernel<SCHEME_B><<<grid, 256, StageCfg<SCHEME_B>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
-  c->launches++;
-  CK(cudaGetLastError());
+  if ((rc = after_launch(c, "stage_kernel"))) return rc;
   return prof_end(c);
 }
 
@@ -233,8 +242,7 @@ int launch_axpy(hard_ctx* c, int stage2, double cfl, double dt_fixed) {
   if (rc) return rc;
   axpy_kernel<<<small_grid(c, N), 256, 0, c->stream>>>(c->U, c->U1, c->Rres, stage2 ? c->U : c->U1, c->g, c->sc, stage2,
                                                         (int)(c->steps_enq & 1), cfl, dt_fixed);
-  c->launches++;
-  CK(cudaGetLastError());
+  if ((rc = after_launch(c, "axpy_kernel"))) return rc;
   return prof_end(c);
 }
 
@@ -331,6 +339,7 @@ hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc) {
   c->g.gamma = gamma;
   c->g.bc = bc;
   c->sm_count = prop.multiProcessorCount;
+  { const char* d = getenv("HARD_DEBUG_SYNC"); c->debug_sync = d && d[0] == '1'; }
   compute_layout(c);
   return c;
 }

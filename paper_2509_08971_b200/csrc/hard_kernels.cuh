@@ -264,8 +264,8 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
   using C = StageCfg<S>;
   constexpr int G = C::G, R = C::R, T = C::T, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS, NIT = C::NIT,
                 XB = C::XB, YB = C::YB;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  double* ring = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double* ring = reinterpret_cast<double*>(smem_raw);   // dynamic smem base is 1024-B aligned (TMA needs 128)
   double* RP = ring + NS * SLOT;       // plus values; overwritten in place by the face fluxes
   double* RM = RP + 5 * NIT;           // minus values
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(RM + 5 * NIT);
