@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py — headline measurement of hard-b200 (contract: see the task statement / DESIGN.md §Measurement).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
+                  [--workload c4|c3|c2s] [--scheme A|B] [--variant fused|perdir]
+
+One "step" = one Heun / SSP-RK2 step of the whole hot path (ghost fill, stage 1, ghost fill, stage 2
+with the fused CFL reduction) over the workload's full mesh.  Metric (BASELINE.json): fp64 cell-updates
+per second per RK stage = cells * 2 * K / time.  Default workload: C4 (BASELINE.json configs[4], 896^3
+periodic seeded sine-mode field, CFL 0.4), scheme A (the paper's WENO5-Z + HLL + Heun).
+N > 1: the path does not shard without a halo exchange that north_star excludes ("everything runs on
+one GPU"), so N ranks run N independent replicas (replicas only), weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 cell-updates/sec per RK stage"
+UNIT = "cell-stage-updates/s"
+ALG_BYTES_PER_CELL_STAGE = 100.0     # stage 1 = 40 R + 40 W, stage 2 = 80 R + 40 W  => 100 B average
+# hand count of the method's minimal fp64 operations per cell-stage (1 FMA = 2 flop)
+ALG_FLOP_PER_CELL_STAGE = {"A": 3240.0, "B": 1010.0}
+
+WORKLOADS = {"c4": (896, 10), "c3": (512, 20), "c2s": (256, 10)}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--scheme", default="A", choices=["A", "B"])
+    ap.add_argument("--variant", default="fused", choices=["fused", "perdir"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for (t, line) in self.rows:
+            if t < t0 or t > t1 + 0.1:
+                continue
+            p = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(p[0]))
+                mx = float(p[1])
+            except Exception:
+                continue
+            for nm, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------ oracle legs
+def oracle_rate(scheme, n, steps, warmup=0):
+    """Times the oracle AS IT STANDS (single-threaded C++) on the same seeded sine-mode recipe at n^3."""
+    import oracle
+    from paper_2509_08971_b200 import workloads as wl
+    w = wl.turbulence(n, nsteps=steps)
+    o = oracle.Oracle(*w.n, w.gamma, w.bc, scheme=0 if scheme == "A" else 1, spacing=w.spacing)
+    o.set_state(*w.state)
+    if warmup:
+        o.step(w.cfl, warmup)
+    t0 = time.perf_counter()
+    o.step(w.cfl, steps)
+    dt = time.perf_counter() - t0
+    o.close()
+    return n ** 3 * 2 * steps / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = 96
+    value, secs = oracle_rate(args.scheme, n, args.steps, args.warmup)
+    sample = ("oracle/hard_oracle.cpp, 1 thread, %d^3 periodic box of the same seeded sine-mode recipe "
+              "(a bounded sample: the full %s mesh needs hours), %d+%d steps" % (n, args.workload, args.warmup, args.steps))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s scheme %s (oracle sample %d^3)" % (args.workload, args.scheme, n)},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------ CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_08971_b200 import hard
+    from paper_2509_08971_b200 import workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    n, _cfg_steps = WORKLOADS[args.workload]
+    K, W = args.steps, args.warmup
+    scheme = hard.SCHEME_WENO5Z_HLL if args.scheme == "A" else hard.SCHEME_MUSCL_HLLC
+    variant = hard.VARIANT_FUSED if args.variant == "fused" else hard.VARIANT_PERDIR
+    w = wl.turbulence(n, nsteps=K, device=dev)
+    cells = n ** 3
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: inputs already in HBM when the timed region starts
+    h.set_state(*w.state)
+    h.step(w.cfl, W)                       # warm-up steps (untimed)
+    h.set_state(*w.state)                  # timed steps are exactly the workload's steps 1..K
+    fp64_peak = hard.probe_fp64_peak()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    launches0 = h.launch_count()
+    h.stage_time(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    e0.record(stream)
+    h.step(w.cfl, K)
+    e1.record(stream)
+    barrier()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    stage_ms, stage_launches = h.stage_time(reset=False)
+    launches = h.launch_count() - launches0
+    clocks = sampler.stop(t0, t1)
+    t_sim, steps_done = h.time()
+    if world > 1:
+        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * cells * 2.0 * K / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (the stage kernel), live CUDA-event durations
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    per_launch_ms = stage_ms / max(stage_launches, 1)
+    if variant == hard.VARIANT_FUSED:
+        cell_stages_per_launch = cells                       # one launch = one RK stage over the mesh
+    else:
+        cell_stages_per_launch = cells * 2.0 * K / max(stage_launches, 1)
+    alg_gbs = cell_stages_per_launch * ALG_BYTES_PER_CELL_STAGE / (per_launch_ms * 1e-3) / 1e9
+    alg_tflops = cell_stages_per_launch * ALG_FLOP_PER_CELL_STAGE[args.scheme] / (per_launch_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "stage_kernel<%s>" % args.scheme, "achieved": alg_tflops, "peak": fp64_peak,
+                "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None, "traffic": None,
+                "peak_source": "measured live: hard_probe_fp64_peak (DFMA chains, all SMs)",
+                "avg_launch_ms": per_launch_ms, "launches_timed": stage_launches,
+                "alg_flop_per_cell_stage": ALG_FLOP_PER_CELL_STAGE[args.scheme]}
+    roofline_hbm = {"bound": "hbm", "achieved": alg_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": alg_gbs / hbm_peak,
+                    "frac_of_nominal_8TBs": alg_gbs / 8000.0, "peak_source": hbm_src,
+                    "alg_bytes_per_cell_stage": ALG_BYTES_PER_CELL_STAGE}
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned): H2D + K steps + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        try:
+            host_in = [torch.empty((n, n, n), dtype=torch.float64, pin_memory=True) for _ in range(5)]
+            for a, b in zip(host_in, w.state):
+                a.copy_(b)
+            host_out = [torch.empty((n, n, n), dtype=torch.float64, pin_memory=True) for _ in range(5)]
+            w.state = None
+            torch.cuda.empty_cache()
+            barrier()
+            te0 = time.perf_counter()
+            h.set_state(*host_in)           # host -> device (5 pitched copies) + CFL pass
+            h.step(w.cfl, K)
+            h.get_state(host_out)           # device -> host, synchronises
+            torch.cuda.synchronize()
+            te = time.perf_counter() - te0
+            if world > 1:
+                tt = torch.tensor([te], device=dev, dtype=torch.float64)
+                dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+                te = float(tt.item())
+            nbytes = 5 * cells * 8
+            e2e = {"value": world * cells * 2.0 * K / te, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+                   "d2h_bytes_per_step": nbytes / K, "seconds": te,
+                   "what": "hard_set_state(host pinned) + hard_step(cfl, %d) + hard_get_state(host pinned); "
+                           "the state crosses PCIe once per %d-step job" % (K, K)}
+            del host_in, host_out
+        except Exception as ex:                      # e.g. not enough pinned host memory on the box
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
+    h.close()
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nb, sb = 128, 3
+        v, secs = oracle_rate(args.scheme, nb, sb)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
+                        "sample": "oracle/hard_oracle.cpp as it stands, 1 thread, %d Heun steps of the same seeded "
+                                  "sine-mode recipe at %d^3 (the %d^3 mesh would take hours)" % (sb, nb, n)}
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "%s: %d^3 periodic seeded sine-mode field, CFL %.2g, %d Heun steps" % (args.workload, n, w.cfl, K),
+                           "scheme": "A: WENO5-Z + HLL + Heun (PAPER.md P:151)" if args.scheme == "A" else "B: MUSCL-minmod + HLLC + SSP-RK2 (north_star fallback)",
+                           "variant": args.variant, "parallelism": "replicas x%d" % world,
+                           "l2": "state (%.1f GB per buffer) is far larger than the 126 MB L2; no flush needed" % (5 * cells * 8 / 1e9),
+                           "sim_time": t_sim, "steps_done": steps_done},
+                "roofline": roofline, "roofline_hbm": roofline_hbm, "e2e": e2e, "cpu_baseline": cpu_baseline,
+                "clocks": clocks, "gpu_launches": launches, "fp64_peak_tflops_measured": fp64_peak}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

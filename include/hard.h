@@ -110,6 +110,12 @@ long long hard_launch_count(const hard_ctx*);
  * since the last call with reset != 0.  Used by bench.py for the roofline of the dominant kernel. */
 int hard_stage_time(hard_ctx*, int reset, double* ms, long long* launches);
 
+/* Measurement utility, not on the hot path: fp64 vector peak of the current device in TFLOP/s
+ * (register-resident DFMA chains on all SMs, best of 4 timed launches).  BASELINE.md §2 / SURVEY.md
+ * Finding 2: the stage kernel is bound by the fp64 pipe, and MEASURED_PEAKS.json has no fp64 entry.
+ * The second argument is reserved (may be NULL). */
+int hard_probe_fp64_peak(double* tflops, double* reserved);
+
 #ifdef __cplusplus
 }
 #endif

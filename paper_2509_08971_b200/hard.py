@@ -22,7 +22,7 @@ VARIANT_FUSED, VARIANT_PERDIR = 0, 1
 EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard_max_dt", "hard_destroy",
            "hard_set_spacing", "hard_set_scheme", "hard_set_variant", "hard_set_stream", "hard_workspace_bytes",
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
-           "hard_stage_time"]
+           "hard_stage_time", "hard_probe_fp64_peak"]
 
 _lib = None
 
@@ -58,8 +58,18 @@ def lib():
     L.hard_launch_count.restype = ctypes.c_longlong
     L.hard_launch_count.argtypes = [vp]
     L.hard_stage_time.argtypes = [vp, c_int, ctypes.POINTER(c_dbl), ctypes.POINTER(ctypes.c_longlong)]
+    L.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(c_dbl), ctypes.POINTER(c_dbl)]
     _lib = L
     return L
+
+
+def probe_fp64_peak():
+    """fp64 vector peak of the current device, TFLOP/s (measurement utility)."""
+    v = ctypes.c_double()
+    rc = lib().hard_probe_fp64_peak(ctypes.byref(v), None)
+    if rc != OK:
+        raise HardError(rc, "hard_probe_fp64_peak")
+    return v.value
 
 
 class HardError(RuntimeError):
