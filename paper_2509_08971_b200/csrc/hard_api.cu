@@ -118,10 +118,10 @@ int make_map(hard_ctx* c, CUtensorMap* m, double* base) {
     fn = (EncodeTiledFn)p;
   }
   const GridDesc& g = c->g;
-  const int T = 16, B = T + 2 * g.g;
+  const int BXh = 14 + 2 * g.g, BYh = 16 + 2 * g.g;          // StageCfg<S>::BX, BY
   cuuint64_t dims[4] = { (cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], 5 };
   cuuint64_t strides[3] = { (cuuint64_t)g.pitch * 8, (cuuint64_t)g.plane * 8, (cuuint64_t)g.fstride * 8 };
-  cuuint32_t box[4] = { (cuuint32_t)B, (cuuint32_t)B, 1, 5 };
+  cuuint32_t box[4] = { (cuuint32_t)BXh, (cuuint32_t)BYh, 1, 5 };
   cuuint32_t es[4] = { 1, 1, 1, 1 };
   CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -135,17 +135,24 @@ int make_map(hard_ctx* c, CUtensorMap* m, double* base) {
 
 int choose_Lz(const hard_ctx* c) {
   const GridDesc& g = c->g;
-  const long long tiles = (long long)((g.n[0] + 15) / 16) * ((g.n[1] + 15) / 16);
+  const long long tiles = (long long)((g.n[0] + 13) / 14) * ((g.n[1] + 15) / 16);
   const int nz = g.n[2];
   if (!g.act[2]) return 1;
+  if (const char* e = getenv("HARD_LZ")) {                   // tuning override (planes per z-chunk)
+    const int v = atoi(e);
+    if (v >= 1) return v < nz ? v : nz;
+  }
+  // cost model (planes of work on the critical path): (waves + 1) * (chunk length + lead-in), where
+  // waves = CTAs / (2 CTAs per SM * SMs) and the +1 is the measured tail of unequal CTA progress
+  // (512^3: one 512-plane chunk per tile = exactly 4 waves ran 15 % slower than 64-plane chunks).
   const double lead = 2.0 + 0.5 * (2 * (g.g - 1) + 1);      // z-only iterations + prologue loads, in plane units
   double best = 1e300;
   int bestc = 1;
   for (int ch = 1; ch <= (nz + 15) / 16; ++ch) {
     const int lz = (nz + ch - 1) / ch;
     const long long ctas = tiles * ((nz + lz - 1) / lz);
-    const double waves = std::ceil((double)ctas / c->sm_count);
-    const double cost = waves * (lz + lead);
+    const double waves = (double)ctas / (2.0 * c->sm_count);
+    const double cost = (waves + 1.0) * (lz + lead);
     if (cost < best * 0.999) { best = cost; bestc = ch; }
   }
   return (nz + bestc - 1) / bestc;
@@ -225,7 +232,7 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
   a.cfl = cfl; a.dt_fixed = dt_fixed;
   const bool zact = g.act[2] && (dirmask & 4);
   a.Lz = zact ? c->Lz : (g.n[2] + ((g.n[2] + 63) / 64) - 1) / ((g.n[2] + 63) / 64);   // z inactive: chunks of <= 64 planes
-  dim3 grid((g.n[0] + 15) / 16, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
+  dim3 grid((g.n[0] + 13) / 14, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
   int rc = prof_begin(c);
   if (rc) return rc;
   if (c->scheme == HARD_SCHEME_WENO5Z_HLL)

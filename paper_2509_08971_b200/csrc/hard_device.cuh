@@ -29,38 +29,38 @@ __device__ __forceinline__ void cons_to_prim(const double U[5], double gm1, doub
 
 // a3, scheme A (Borges et al. [18]; G1: eps = 1e-40, power 1, d = (1/10, 6/10, 3/10)).
 // Both face values of cell i from q[i-2..i+2] = (a,b,c,d,e): plus at i+1/2, minus at i-1/2.  The
-// minus value is the same function on the mirrored stencil, so the smoothness indicators and
-// tau/(beta+eps) ratios are shared: beta0' = beta2, beta1' = beta1, beta2' = beta0.
+// minus value is the same function on the mirrored stencil, so the smoothness indicators are shared
+// (beta0' = beta2, beta1' = beta1, beta2' = beta0).  Algebraically identical to the definition, but
+// arranged for the fp64 pipe:
+//  * everything in terms of the four differences d1..d4 (candidates minus c are 2-term forms);
+//  * beta scaled by 12/13 (beta' = s^2 + 3/13 t^2, eps' = 12/13 eps): tau/(beta+eps) is unchanged;
+//  * weights d_k (1 + tau/B_k) multiplied through by B0 B1 B2: d_k (B_k + tau) prod_{j!=k} B_j, which
+//    needs no division; ONE reciprocal 1/(sp*sm) normalises both sides.
+//    Range: B in [9e-41, ~1e17] for admissible data of the configs, so products of three B's and the
+//    square of their sum stay within [1e-241, 1e110]: no overflow / underflow in fp64.
 __device__ __forceinline__ void wenoz_pair(double a, double b, double c, double d, double e, double& plus,
                                            double& minus) {
-  const double eps = 1e-40;
-  const double s0 = (a - 2.0 * b) + c, t0 = (a - 4.0 * b) + 3.0 * c;
-  const double s1 = (b - 2.0 * c) + d, t1 = b - d;
-  const double s2 = (c - 2.0 * d) + e, t2 = (3.0 * c - 4.0 * d) + e;
-  const double b0 = (13.0 / 12.0) * (s0 * s0) + 0.25 * (t0 * t0);
-  const double b1 = (13.0 / 12.0) * (s1 * s1) + 0.25 * (t1 * t1);
-  const double b2 = (13.0 / 12.0) * (s2 * s2) + 0.25 * (t2 * t2);
-  const double tau = fabs(b0 - b2);
-  // r_k = tau / (beta_k + eps) with ONE reciprocal: 1/(B0 B1 B2).  beta <= ~1e17 for admissible
-  // data of the configs, eps^3 = 1e-120: no overflow / underflow in fp64.
-  const double B0 = b0 + eps, B1 = b1 + eps, B2 = b2 + eps;
-  const double B01 = B0 * B1;
-  const double ti = tau * (1.0 / (B01 * B2));
-  const double r0 = ti * (B1 * B2), r1 = ti * (B0 * B2), r2 = ti * B01;
-  const double q0 = (1.0 / 6.0) * ((2.0 * a - 7.0 * b) + 11.0 * c);
-  const double q1 = (1.0 / 6.0) * ((5.0 * c - b) + 2.0 * d);
-  const double q2 = (1.0 / 6.0) * ((2.0 * c + 5.0 * d) - e);
-  const double p0 = (1.0 / 6.0) * ((2.0 * e - 7.0 * d) + 11.0 * c);
-  const double p1 = (1.0 / 6.0) * ((5.0 * c - d) + 2.0 * b);
-  const double p2 = (1.0 / 6.0) * ((2.0 * c + 5.0 * b) - a);
-  const double a0 = fma(0.1, r0, 0.1), a1 = fma(0.6, r1, 0.6), a2 = fma(0.3, r2, 0.3);   // plus
-  const double m0 = fma(0.1, r2, 0.1), m1 = a1, m2 = fma(0.3, r0, 0.3);                  // minus
-  const double sp = (a0 + a1) + a2, sm = (m0 + m1) + m2;
-  const double np = (a0 * q0 + a1 * q1) + a2 * q2;
-  const double nm = (m0 * p0 + m1 * p1) + m2 * p2;
-  const double inv = 1.0 / (sp * sm);                     // sp, sm in [1, ~1e57]: safe
-  plus = np * (inv * sm);
-  minus = nm * (inv * sp);
+  const double eps = (12.0 / 13.0) * 1e-40, k3 = 3.0 / 13.0;
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  const double s0 = d2 - d1, s1 = d3 - d2, s2 = d4 - d3;
+  const double t0 = fma(3.0, d2, -d1), t1 = d2 + d3, t2 = fma(-3.0, d3, d4);
+  const double B0 = fma(s0, s0, fma(k3 * t0, t0, eps));
+  const double B1 = fma(s1, s1, fma(k3 * t1, t1, eps));
+  const double B2 = fma(s2, s2, fma(k3 * t2, t2, eps));
+  const double tau = fabs(B0 - B2);
+  const double P12 = B1 * B2, P02 = B0 * B2, P01 = B0 * B1;
+  const double T0 = B0 + tau, T1 = B1 + tau, T2 = B2 + tau;
+  const double a0 = (0.1 * T0) * P12, a1 = (0.6 * T1) * P02, a2 = (0.3 * T2) * P01;   // plus weights
+  const double m0 = (0.1 * T2) * P01, m2 = (0.3 * T0) * P12;                           // minus (m1 = a1)
+  const double sp = (a0 + a1) + a2, sm = (m0 + a1) + m2;
+  // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
+  const double q0 = fma(5.0, d2, -2.0 * d1), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);
+  const double p0 = fma(-5.0, d3, 2.0 * d4), p1 = -fma(2.0, d2, d3), p2 = fma(-4.0, d2, d1);
+  const double np = fma(a2, q2, fma(a1, q1, a0 * q0));
+  const double nm = fma(m2, p2, fma(a1, p1, m0 * p0));
+  const double inv6 = (1.0 / 6.0) / (sp * sm);
+  plus = fma(np, inv6 * sm, c);
+  minus = fma(nm, inv6 * sp, c);
 }
 
 // a3, scheme B: MUSCL with the minmod limiter, sign tests (no product).
@@ -78,8 +78,10 @@ __device__ __forceinline__ void minmod_pair(double b, double c, double d, double
 template <int S>
 __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR[5], double gamma, double inv_gm1,
                                              double F[5]) {
-  const double cL = sqrt(gamma * WL[4] / WL[0]);
-  const double cR = sqrt(gamma * WR[4] / WR[0]);
+  // c = sqrt(gamma p / rho) = gamma p * rsqrt(gamma p rho): no division (rsqrt: <= 1 ulp)
+  const double gpL = gamma * WL[4], gpR = gamma * WR[4];
+  const double cL = gpL * rsqrt(gpL * WL[0]);
+  const double cR = gpR * rsqrt(gpR * WR[0]);
   const double SL = fmin(WL[1] - cL, WR[1] - cR);
   const double SR = fmax(WL[1] + cL, WR[1] + cR);
   const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));

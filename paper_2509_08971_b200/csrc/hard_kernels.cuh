@@ -219,24 +219,33 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
 }
 
 // ------------------------------------------------------------------------------------------- a2..a7 fused stage
+// One CTA = a 14 x 16 (x, y) tile of cells marched along z; 256 threads laid out 16 x 16:
+//   x: thread (tx, ty) reconstructs cell ix = tx-1 (-1..14) of row ty; the minus value of the right
+//      neighbour and the flux of the left face travel by warp shuffles inside the 16-lane row
+//      segment: no shared-memory exchange, no barrier.  Threads tx = 1..14 own cells 0..13.
+//   y: 14 x 18 = 252 items (cells iy = -1..16) through shared memory (minus values, then fluxes).
+//   z: each owner thread marches its own column: the plus value and the flux of the previous plane
+//      stay in registers; the z stencil is read from a ring of primitive planes in shared memory.
+// Every face flux and every cell reconstruction inside a tile is computed once; 224 of 256 lanes do
+// useful work in every phase.  The ring holds conserved planes loaded by TMA (4-D box: x, y, one z
+// plane, five fields) and converted to primitives in place (a2).
 template <int S>
 struct StageCfg {
   static constexpr int G = SchemeTraits<S>::G, R = SchemeTraits<S>::R;
-  static constexpr int T = 16;                         // x-y tile edge (cells); 256 threads, one per cell
-  static constexpr int NT = T * T;
-  static constexpr int BX = T + 2 * G, BY = T + 2 * G; // TMA box
-  static constexpr int VS = BX * BY;                   // doubles per field per plane slot
-  static constexpr int SLOT = (5 * VS + 15) / 16 * 16; // slot stride, multiple of 128 B
-  static constexpr int NS = 2 * R + 2;                 // ring: z window 2R+1 plus one plane in flight
-  static constexpr int NXI = (T + 2) * T;              // x (or y) reconstruction items per plane
-  static constexpr int XB = NT, YB = NT + NXI;         // item bases: [z | x | y]
-  static constexpr int NIT = NT + 2 * NXI;
+  static constexpr int TX = 14, TY = 16, NT = 256;
+  static constexpr int BX = TX + 2 * G, BY = TY + 2 * G;      // TMA box
+  static constexpr int VS = BX * BY;                          // doubles per field per plane slot
+  static constexpr int SLOT = (5 * VS + 15) / 16 * 16;        // slot stride, multiple of 128 B
+  // z window of 2R+1 planes.  R >= 2: the oldest plane is not the x/y plane, it is released after the
+  // z reconstruction and its slot takes the next plane (no spare slot); otherwise one spare slot.
+  static constexpr int NS = (R >= 2) ? 2 * R + 1 : 2 * R + 2;
+  static constexpr int NYI = TX * (TY + 2);                   // y reconstruction items
   static constexpr uint32_t BOX_BYTES = 5u * VS * 8u;
-  static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * 5 * NIT * 8 + NS * 8 + 64 * 8 + 128;
+  static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * 5 * NYI * 8 + NS * 8 + 64 * 8;
 };
 
-// Reconstruct both face values of all five primitives of one item (cell + direction).
-// o[s] = ring offset (doubles) of field 0 at stencil position s - R.
+// Both face values of all five primitives of one cell along one direction; o[s] = ring offset of
+// field 0 at stencil position s - R.  Scheme A applies the positivity fallback (G4).
 template <int S>
 __device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double pl[5], double mi[5]) {
   constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S>::VS;
@@ -249,7 +258,7 @@ __device__ __forceinline__ void recon_item(const double* __restrict__ ring, cons
       minmod_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], pl[v], mi[v]);
     }
   }
-  if (S == SCHEME_A) {                                   // G4 positivity fallback: piecewise constant
+  if (S == SCHEME_A) {
     if (pl[0] <= 0.0 || pl[4] <= 0.0 || mi[0] <= 0.0 || mi[4] <= 0.0) {
 #pragma unroll
       for (int v = 0; v < 5; ++v) pl[v] = mi[v] = ring[o[R] + v * VS];
@@ -257,35 +266,51 @@ __device__ __forceinline__ void recon_item(const double* __restrict__ ring, cons
   }
 }
 
+// Flux through a face with normal along direction D from (rho,u,v,w,p) face states; result in
+// (rho, mx, my, mz, E) order.
+template <int S, int D>
+__device__ __forceinline__ void face_flux(const double L[5], const double Rr[5], double gamma, double inv_gm1,
+                                          double F[5]) {
+  constexpr int n = 1 + D, t1 = 1 + (D + 1) % 3, t2 = 1 + (D + 2) % 3;
+  const double WL[5] = { L[0], L[n], L[t1], L[t2], L[4] };
+  const double WR[5] = { Rr[0], Rr[n], Rr[t1], Rr[t2], Rr[4] };
+  double f[5];
+  riemann_flux<S>(WL, WR, gamma, inv_gm1, f);
+  F[0] = f[0]; F[n] = f[1]; F[t1] = f[2]; F[t2] = f[3]; F[4] = f[4];
+}
+
 template <int S>
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(256, 2)
 stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict__ Usrc, const double* Uaux,
              double* Uout, GridDesc g, DevScalars* sc, StageArgs a) {
   using C = StageCfg<S>;
-  constexpr int G = C::G, R = C::R, T = C::T, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS, NIT = C::NIT,
-                XB = C::XB, YB = C::YB;
+  constexpr int G = C::G, R = C::R, TX = C::TX, TY = C::TY, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS,
+                NYI = C::NYI;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);   // dynamic smem base is 1024-B aligned (TMA needs 128)
-  double* RP = ring + NS * SLOT;       // plus values; overwritten in place by the face fluxes
-  double* RM = RP + 5 * NIT;           // minus values
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(RM + 5 * NIT);
+  double* RMy = ring + NS * SLOT;      // y minus values, item-indexed [v][item]
+  double* Fy = RMy + 5 * NYI;          // y face fluxes: item's upper face
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + 5 * NYI);
   double* red = reinterpret_cast<double*>(bars + NS);
 
-  const int tid = threadIdx.x, tx = tid & (T - 1), ty = tid / T;
-  const int i0 = blockIdx.x * T, j0 = blockIdx.y * T, k0 = blockIdx.z * a.Lz;
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, k0 = blockIdx.z * a.Lz;
   const int kend = min(g.n[2], k0 + a.Lz);
   const bool ax = g.act[0] && (a.dirmask & 1), ay = g.act[1] && (a.dirmask & 2), az = g.act[2] && (a.dirmask & 4);
-  const int rows = min(T, g.n[1] - j0), cols = min(T, g.n[0] - i0);
-  const bool mine = tx < cols && ty < rows;
+  const int rows = min(TY, g.n[1] - j0), cols = min(TX, g.n[0] - i0);
+  const bool mine = tx >= 1 && tx <= cols && ty < rows;          // thread tx owns cell ix = tx - 1
+  const bool yitem = ay && tid < TX * (rows + 2), yface = ay && tid < TX * (rows + 1);
+  const int y_c = tid / TX, y_ix = tid - y_c * TX;               // y item: cell (y_ix, y_c - 1)
   const double gamma = g.gamma, gm1 = gamma - 1.0, inv_gm1 = 1.0 / gm1;
   const double dt = step_dt(sc, a.cur, a.cfl, a.dt_fixed);
+  const double idx = g.inv_d[0], idy = g.inv_d[1], idz = g.inv_d[2];
 
   // z window of iteration kk: planes [kk + ld - rz, kk + ld + rz]; with z active the z stencil runs
   // one plane ahead so that both z faces of plane kk are known when its x/y fluxes are.
   const int ld = az ? 1 : 0, rz = az ? R : 0;
   const int kfirst = az ? k0 - 2 : k0;
   const int zb = kfirst + ld - rz;                     // first plane ever loaded; ring slot = (z - zb) % NS
-  const int cx = g.off[0] + i0 - G, cy = g.off[1] + j0 - G;
+  const int cx = g.off[0] + i0 - G, cy = g.off[1] + j0 - G;      // cx = i0: even, so 16-byte aligned
 
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) mbar_init(smem_u32(&bars[s]), 1);
@@ -318,7 +343,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
   for (int z = zb; z <= zb + 2 * rz; ++z) wait_convert(z);
   __syncthreads();
 
-  double zplus[5] = { 0, 0, 0, 0, 0 }, Fzold[5] = { 0, 0, 0, 0, 0 }, Fznew[5] = { 0, 0, 0, 0, 0 };
+  double zplus[5] = { 0, 0, 0, 0, 0 }, Fzold[5] = { 0, 0, 0, 0, 0 };
   double lam_loc = 0.0;
   int bad = 0;
   const bool act3[3] = { g.act[0] != 0, g.act[1] != 0, g.act[2] != 0 };
@@ -327,15 +352,50 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     const bool doxy = kk >= k0;
     const int znext = kk + 1 + ld + rz;
     const bool more = kk + 1 < kend;
-    if (more && tid == 0) {                            // prefetch the plane the next iteration adds
-      fence_proxy_async();                             // its slot was last touched by generic-proxy accesses
-      issue(znext);
+    // the slot of the next plane still holds the oldest plane of this window (no spare slot): it is
+    // released by the barrier after the z reconstruction
+    const bool late = (znext - NS) >= (kk + ld - rz);
+    if (more && !late && tid == 0) { fence_proxy_async(); issue(znext); }
+    const int slot_c = ((kk - zb) % NS) * SLOT;        // plane kk (x/y stencils)
+    double Lacc[5] = { 0, 0, 0, 0, 0 };                 // L(U) of the owned cell, accumulated in registers (a5)
+
+    // ---- z: reconstruct plane kk+1 (own column), flux through face kk+1/2 with the carried plus value
+    if (az) {
+      int o[2 * R + 1];
+      const int cell = (ty + G) * BX + (tx - 1 + G);
+#pragma unroll
+      for (int s = -R; s <= R; ++s) o[s + R] = ((kk + 1 + s - zb) % NS) * SLOT + cell;
+      double pl[5], mi[5];
+      recon_item<S>(ring, o, pl, mi);
+      if (kk >= k0 - 1) {
+        double F[5];
+        face_flux<S, 2>(zplus, mi, gamma, inv_gm1, F);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) { Lacc[v] = (Fzold[v] - F[v]) * idz; Fzold[v] = F[v]; }
+      }
+#pragma unroll
+      for (int v = 0; v < 5; ++v) zplus[v] = pl[v];
     }
+    // ---- y: reconstruct the 14 x (rows+2) items of plane kk; minus values to shared memory
+    double plY[5] = { 0, 0, 0, 0, 0 };
+    if (doxy && yitem) {
+      int o[2 * R + 1];
+      const int cell = slot_c + (y_c - 1 + G) * BX + (y_ix + G);
+#pragma unroll
+      for (int s = -R; s <= R; ++s) o[s + R] = cell + s * BX;
+      double mi[5];
+      recon_item<S>(ring, o, plY, mi);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) RMy[v * NYI + tid] = mi[v];
+    }
+    __syncthreads();                                                             // barrier 1
+    if (more && late && tid == 0) { fence_proxy_async(); issue(znext); }
+
     // own-cell conserved values for the RK combination: issued now, consumed after the flux phases
     double uc[5] = { 0, 0, 0, 0, 0 }, ua[5] = { 0, 0, 0, 0, 0 };
     long long pc = 0;
     if (doxy && mine) {
-      pc = cell_addr(g, i0 + tx, j0 + ty, kk);
+      pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
       if (a.mode != MODE_RESID) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) uc[v] = Usrc[v * g.fstride + pc];
@@ -345,86 +405,44 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
         for (int v = 0; v < 5; ++v) ua[v] = Uaux[v * g.fstride + pc];
       }
     }
-
-    // ---- a3: reconstruction items [z: own cell of plane kk+1 | x: (T+2) x rows | y: T x (rows+2)]
-    const int slot_c = ((kk - zb) % NS) * SLOT;        // plane kk (x/y stencils)
-    const int L0 = az ? C::NT : 0;
-    const int L1 = L0 + ((doxy && ax) ? (T + 2) * rows : 0);
-    const int L2 = L1 + ((doxy && ay) ? T * (rows + 2) : 0);
-    for (int it = tid; it < L2; it += C::NT) {
-      int o[2 * R + 1], st;
-      if (it < L0) {
-        st = it;
-        const int cell = (ty + G) * BX + (tx + G);
-#pragma unroll
-        for (int s = -R; s <= R; ++s) o[s + R] = ((kk + 1 + s - zb) % NS) * SLOT + cell;
-      } else if (it < L1) {
-        const int j = it - L0, row = j / (T + 2), c = j - row * (T + 2);
-        st = XB + j;
-        const int cell = slot_c + (row + G) * BX + (c - 1 + G);
+    // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
+    if (doxy && ax) {
+      double pl[5] = { 1, 0, 0, 0, 1 }, mi[5] = { 1, 0, 0, 0, 1 }, mr[5], F[5];
+      if (ty < rows) {
+        int o[2 * R + 1];
+        const int cell = slot_c + (ty + G) * BX + (tx - 1 + G);
 #pragma unroll
         for (int s = -R; s <= R; ++s) o[s + R] = cell + s;
-      } else {
-        const int j = it - L1, c = j / T, ix = j - c * T;
-        st = YB + j;
-        const int cell = slot_c + (c - 1 + G) * BX + (ix + G);
-#pragma unroll
-        for (int s = -R; s <= R; ++s) o[s + R] = cell + s * BX;
-      }
-      double pl[5], mi[5];
-      recon_item<S>(ring, o, pl, mi);
-#pragma unroll
-      for (int v = 0; v < 5; ++v) { RP[v * NIT + st] = pl[v]; RM[v * NIT + st] = mi[v]; }
-    }
-    __syncthreads();
-
-    // ---- a4: each face flux once.  z face kk+1/2 in registers (left state carried from the
-    // previous plane); x / y faces from the item arrays, flux written over the left item's plus slot.
-    if (az) {
-      if (kk >= k0 - 1) {
-        const double WL[5] = { zplus[0], zplus[3], zplus[1], zplus[2], zplus[4] };          // (n,t1,t2) = (w,u,v)
-        const double WR[5] = { RM[0 * NIT + tid], RM[3 * NIT + tid], RM[1 * NIT + tid], RM[2 * NIT + tid],
-                               RM[4 * NIT + tid] };
-        double F[5];
-        riemann_flux<S>(WL, WR, gamma, inv_gm1, F);
-        Fznew[0] = F[0]; Fznew[3] = F[1]; Fznew[1] = F[2]; Fznew[2] = F[3]; Fznew[4] = F[4];
+        recon_item<S>(ring, o, pl, mi);
       }
 #pragma unroll
-      for (int v = 0; v < 5; ++v) zplus[v] = RP[v * NIT + tid];
-    }
-    if (doxy) {
-      const int nxf = ax ? (T + 1) * rows : 0;
-      const int nyf = ay ? T * (rows + 1) : 0;
-      for (int it = tid; it < nxf + nyf; it += C::NT) {
-        int Li, Ri, d;
-        if (it < nxf) {
-          const int row = it / (T + 1), c = it - row * (T + 1);
-          Li = XB + row * (T + 2) + c; Ri = Li + 1; d = 0;
-        } else {
-          const int j = it - nxf;
-          Li = YB + j; Ri = Li + T; d = 1;
-        }
-        const int vn = 1 + d, vt1 = 1 + (d + 1) % 3, vt2 = 1 + (d + 2) % 3;
-        const double WL[5] = { RP[Li], RP[vn * NIT + Li], RP[vt1 * NIT + Li], RP[vt2 * NIT + Li], RP[4 * NIT + Li] };
-        const double WR[5] = { RM[Ri], RM[vn * NIT + Ri], RM[vt1 * NIT + Ri], RM[vt2 * NIT + Ri], RM[4 * NIT + Ri] };
-        double F[5];
-        riemann_flux<S>(WL, WR, gamma, inv_gm1, F);
-        RP[Li] = F[0]; RP[vn * NIT + Li] = F[1]; RP[vt1 * NIT + Li] = F[2]; RP[vt2 * NIT + Li] = F[3];
-        RP[4 * NIT + Li] = F[4];
-      }
-    }
-    __syncthreads();
-
-    // ---- a5 + a6 (+ a7): divergence in registers, RK combination, store
-    if (doxy && mine) {
-      double out[5];
-      const int xi = XB + ty * (T + 2) + tx, yi = YB + ty * T + tx;
+      for (int v = 0; v < 5; ++v) mr[v] = __shfl_down_sync(0xffffffffu, mi[v], 1, 16);   // minus of cell tx
+      face_flux<S, 0>(pl, mr, gamma, inv_gm1, F);                                        // face right of cell tx-1
 #pragma unroll
       for (int v = 0; v < 5; ++v) {
-        double L = 0.0;
-        if (ax) L -= (RP[v * NIT + xi + 1] - RP[v * NIT + xi]) * g.inv_d[0];
-        if (ay) L -= (RP[v * NIT + yi + T] - RP[v * NIT + yi]) * g.inv_d[1];
-        if (az) L -= (Fznew[v] - Fzold[v]) * g.inv_d[2];
+        const double Fl = __shfl_up_sync(0xffffffffu, F[v], 1, 16);                      // face left of cell tx-1
+        Lacc[v] -= (F[v] - Fl) * idx;
+      }
+    }
+    // ---- y fluxes: face above item (between item and item + TX)
+    if (doxy && yface) {
+      double mr[5], F[5];
+#pragma unroll
+      for (int v = 0; v < 5; ++v) mr[v] = RMy[v * NYI + tid + TX];
+      face_flux<S, 1>(plY, mr, gamma, inv_gm1, F);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) Fy[v * NYI + tid] = F[v];
+    }
+    __syncthreads();                                                             // barrier 2
+
+    // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
+    if (doxy && mine) {
+      double out[5];
+      const int yi = ty * TX + (tx - 1);               // item of cell (tx-1, ty-1): its upper face is our lower face
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        double L = Lacc[v];
+        if (ay) L -= (Fy[v * NYI + yi + TX] - Fy[v * NYI + yi]) * idy;
         if (a.mode == MODE_STAGE1) out[v] = fma(dt, L, uc[v]);
         else if (a.mode == MODE_STAGE2) out[v] = 0.5 * ua[v] + 0.5 * fma(dt, L, uc[v]);
         else out[v] = a.first ? L : ua[v] + L;
@@ -435,12 +453,8 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
         if (l < 0.0) bad = 1; else lam_loc = fmax(lam_loc, l);
       }
     }
-    if (az) {
-#pragma unroll
-      for (int v = 0; v < 5; ++v) Fzold[v] = Fznew[v];
-    }
     if (more) wait_convert(znext);
-    __syncthreads();
+    __syncthreads();                                                             // barrier 3
   }
   if (a.mode == MODE_STAGE2) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
 }
