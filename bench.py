@@ -29,7 +29,8 @@ METRIC = "fp64 cell-updates/sec per RK stage"
 UNIT = "cell-stage-updates/s"
 ALG_BYTES_PER_CELL_STAGE = 100.0     # stage 1 = 40 R + 40 W, stage 2 = 80 R + 40 W  => 100 B average
 # hand count of the method's minimal fp64 operations per cell-stage (1 FMA = 2 flop)
-ALG_FLOP_PER_CELL_STAGE = {"A": 3240.0, "B": 1010.0}
+# (A: 1300, B: 540 fp64-pipe instructions; 2 flop-equivalents each, the DFMA peak's own unit)
+ALG_FLOP_PER_CELL_STAGE = {"A": 2600.0, "B": 1080.0}
 
 WORKLOADS = {"c4": (896, 10), "c3": (512, 20), "c2s": (256, 10)}
 
@@ -46,6 +47,23 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------ ranks
+def max_over_ranks(x, device="cpu"):
+    """Max of a python float over all ranks (identity when torch.distributed is not initialised)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(cells_per_rank, stages, steps, ms_max, world):
+    """Whole-job cell-stage-updates/s of `world` replicas that each did cells*stages*steps in ms_max."""
+    return world * cells_per_rank * float(stages) * steps / (ms_max * 1e-3)
 
 
 # ------------------------------------------------------------------------------------ clocks
@@ -186,11 +204,8 @@ def run_cuda(args):
     launches = h.launch_count() - launches0
     clocks = sampler.stop(t0, t1)
     t_sim, steps_done = h.time()
-    if world > 1:
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    value = world * cells * 2.0 * K / (ms * 1e-3)
+    ms = max_over_ranks(ms, dev)
+    value = job_throughput(cells, 2, K, ms, world)
 
     # ---- roofline of the dominant kernel (the stage kernel), live CUDA-event durations
     peaks = {}
@@ -233,12 +248,9 @@ def run_cuda(args):
             h.get_state(host_out)           # device -> host, synchronises
             torch.cuda.synchronize()
             te = time.perf_counter() - te0
-            if world > 1:
-                tt = torch.tensor([te], device=dev, dtype=torch.float64)
-                dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-                te = float(tt.item())
+            te = max_over_ranks(te, dev)
             nbytes = 5 * cells * 8
-            e2e = {"value": world * cells * 2.0 * K / te, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+            e2e = {"value": job_throughput(cells, 2, K, te * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
                    "d2h_bytes_per_step": nbytes / K, "seconds": te,
                    "what": "hard_set_state(host pinned) + hard_step(cfl, %d) + hard_get_state(host pinned); "
                            "the state crosses PCIe once per %d-step job" % (K, K)}
