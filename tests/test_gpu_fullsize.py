@@ -1,0 +1,129 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (-m gpu).
+
+C2 (Sedov 128^3): full-domain oracle for 1 and 12 steps.  C3 (512^3) / C4 (896^3): the full-domain oracle
+would need hours, so parity uses the light-cone sub-box oracle of DESIGN.md §3: a (B + 2 s 2g)^3 block of
+the initial state (periodic wrap) is stepped by the oracle with the GPU's dt sequence and zero-gradient
+ghosts; their error travels 2g cells per step, so the central B^3 is bit-identical to what a full-domain
+oracle would give.  dt at step 0 is checked against the oracle run on the z-slab that holds the
+maximum-wavespeed cell."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2509_08971_b200 import hard
+from paper_2509_08971_b200 import workloads as wl
+
+from _parity import field_errors, run_both
+
+pytestmark = pytest.mark.gpu
+TOL_1, TOL_100, TOL_DT = 1e-12, 1e-9, 1e-14
+
+
+@pytest.mark.parametrize("scheme,nsteps", [(hard.SCHEME_WENO5Z_HLL, 1), (hard.SCHEME_WENO5Z_HLL, 12),
+                                           (hard.SCHEME_MUSCL_HLLC, 1), (hard.SCHEME_MUSCL_HLLC, 12)])
+def test_sedov_c2_full_domain(scheme, nsteps):
+    w = wl.sedov(128)
+    g, o, dts, ts, dte = run_both(w, scheme, hard.VARIANT_FUSED, nsteps=nsteps)
+    assert abs(dts[0] - dts[1]) <= TOL_DT * dts[1]
+    assert max(field_errors(g, o)) <= (TOL_1 if nsteps == 1 else TOL_100)
+    assert abs(ts[0] - ts[1]) <= 1e-12 * ts[1]
+
+
+def _subbox(state, lo, size):
+    """Periodic (wrapping) cube of edge `size` with low corner `lo` (x,y,z) out of device tensors (z,y,x)."""
+    import torch
+    n = state[0].shape[0]
+    dev = state[0].device
+    ix = [(torch.arange(size, device=dev) + lo[a]) % n for a in range(3)]
+    out = []
+    for f in state:
+        b = f.index_select(0, ix[2]).index_select(1, ix[1]).index_select(2, ix[0])
+        out.append(np.ascontiguousarray(b.cpu().numpy()))
+    return out
+
+
+def _check_subboxes(n, scheme, boxes, B, device_state, w):
+    """boxes: list of (low corner of the central B^3 cube, steps s)."""
+    g = 3 if scheme == hard.SCHEME_WENO5Z_HLL else 2
+    smax = max(s for _, s in boxes)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+    h.set_state(*device_state)
+    # the GPU runs hard_step(cfl, 1) per step exactly as bench.py's hard_step(cfl, K) does; dt_i is read back
+    dts, snaps = [], {}
+    need = sorted(set(s for _, s in boxes))
+    import torch
+    for i in range(smax):
+        dts.append(w.cfl * h.max_dt())
+        h.step(w.cfl, 1)
+        if i + 1 in need:
+            out = [torch.empty_like(a) for a in device_state]
+            h.get_state(out)
+            snaps[i + 1] = out
+    t, steps = h.time()
+    assert steps == smax and abs(t - sum(dts)) <= 1e-13 * t
+    h.close()
+    worst = 0.0
+    for lo, s in boxes:
+        m = s * 2 * g
+        size = B + 2 * m
+        init = _subbox(device_state, [c - m for c in lo], size)
+        o = oracle.Oracle(size, size, size, w.gamma, wl.BC_OUTFLOW, scheme=scheme, spacing=w.spacing, check=False)
+        o.set_state(*init)
+        for i in range(s):
+            o.step_dt(dts[i], 1)
+        ref = [a[m:m + B, m:m + B, m:m + B] for a in o.get_state()]
+        o.close()
+        got = _subbox(snaps[s], lo, B)
+        errs = field_errors(got, ref)
+        tol = TOL_1 if s == 1 else TOL_100
+        assert max(errs) <= tol, "box %s after %d steps: %s" % (lo, s, errs)
+        assert all(np.abs(a - b[m:m + B, m:m + B, m:m + B]).max() > 0 for a, b in zip(ref[:1], init[:1]))
+        worst = max(worst, max(errs))
+    return worst
+
+
+def _dt0_check(n, scheme, device_state, w):
+    """lambda of the full mesh = lambda of the z-slab holding the max-wavespeed cell (max is exact)."""
+    import torch
+    rho, mx, my, mz, E = device_state
+    best, kbest = -1.0, 0
+    for k0 in range(0, n, 32):
+        sl = slice(k0, min(n, k0 + 32))
+        u, v, ww = mx[sl] / rho[sl], my[sl] / rho[sl], mz[sl] / rho[sl]
+        p = (w.gamma - 1.0) * (E[sl] - 0.5 * (mx[sl] * u + my[sl] * v + mz[sl] * ww))
+        c = torch.sqrt(w.gamma * p / rho[sl])
+        lam = float(((torch.maximum(torch.maximum(u.abs(), v.abs()), ww.abs()) + c) / w.spacing[0]).max())
+        if lam > best:
+            best, kbest = lam, k0
+    slab = [np.ascontiguousarray(a[kbest:kbest + 32].cpu().numpy()) for a in device_state]
+    o = oracle.Oracle(n, n, slab[0].shape[0], w.gamma, wl.BC_PERIODIC, scheme=scheme, spacing=w.spacing)
+    o.set_state(*slab)
+    dt_orc = o.max_dt()
+    o.close()
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+    h.set_state(*device_state)
+    dt_gpu = h.max_dt()
+    h.close()
+    assert abs(dt_gpu - dt_orc) <= TOL_DT * dt_orc
+    assert abs(1.0 / dt_orc - best) <= 1e-12 * best
+
+
+@pytest.mark.parametrize("n,scheme,long_steps,Blong", [(512, hard.SCHEME_WENO5Z_HLL, 10, 16),
+                                                      (512, hard.SCHEME_MUSCL_HLLC, 20, 8),
+                                                      (896, hard.SCHEME_WENO5Z_HLL, 10, 16),
+                                                      (896, hard.SCHEME_MUSCL_HLLC, 10, 16)])
+def test_throughput_configs_c3_c4_lightcone(n, scheme, long_steps, Blong):
+    import torch
+    w = wl.turbulence(n, device="cuda")
+    state = w.state
+    _dt0_check(n, scheme, state, w)
+    rng = np.random.default_rng(n + scheme)
+    B = 24
+    one_step = [([n - 10, n - 7, n - 12], 1),                     # straddles the periodic seam in x, y and z
+                ([n // 2, n // 2, n // 2], 1),
+                ([int(rng.integers(0, n)) for _ in range(3)], 1),
+                ([13 * 14 - 5, 3 * 16 - 9, 224 - 11], 1)]          # straddles tile and z-chunk boundaries
+    _check_subboxes(n, scheme, one_step, B, state, w)
+    _check_subboxes(n, scheme, [([n - 6, n - 5, n - 7], long_steps)], Blong, state, w)
+    del state, w
+    torch.cuda.empty_cache()
