@@ -29,6 +29,18 @@ __device__ __forceinline__ double fast_rcp(double x) {
   return fma(y, e, y);
 }
 
+// 1/sqrt(x) for normal, finite x > 0: MUFU.RSQ64H seed + two Newton steps (7 fp64-pipe instructions,
+// about 1 ulp), no special-case handling.
+__device__ __forceinline__ double fast_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * x;
+  double e = fma(-h, y * y, 0.5);
+  y = fma(y, e, y);
+  e = fma(-h, y * y, 0.5);
+  return fma(y, e, y);
+}
+
 // a2 (eq.2): (rho, mx, my, mz, E) -> (rho, u, v, w, p).
 __device__ __forceinline__ void cons_to_prim(const double U[5], double gm1, double W[5]) {
   const double inv = fast_rcp(U[0]);
@@ -75,12 +87,16 @@ __device__ __forceinline__ void wenoz_pair(double a, double b, double c, double 
   minus = fma(nm, inv6 * sp, c);
 }
 
-// a3, scheme B: MUSCL with the minmod limiter, sign tests (no product).
+// a3, scheme B: MUSCL with the minmod limiter.  Branch-free: the slope is min(|x|,|y|) with the sign
+// of x when x and y have the same sign (test on the sign bits, integer pipe) and 0 otherwise —
+// the same value as the sign-test definition for all finite inputs (x or y = 0 gives 0).
 __device__ __forceinline__ void minmod_pair(double b, double c, double d, double& plus, double& minus) {
   const double x = c - b, y = d - c;
-  double s = 0.0;
-  if (x > 0.0 && y > 0.0) s = fmin(x, y);
-  else if (x < 0.0 && y < 0.0) s = fmax(x, y);
+  const double m = fmin(fabs(x), fabs(y));
+  const int hx = __double2hiint(x), hy = __double2hiint(y);
+  const int hm = ((hx ^ hy) < 0) ? 0 : (__double2hiint(m) | (hx & 0x80000000));
+  const int lm = ((hx ^ hy) < 0) ? 0 : __double2loint(m);
+  const double s = __hiloint2double(hm, lm);
   plus = fma(0.5, s, c);
   minus = fma(-0.5, s, c);
 }
@@ -90,52 +106,66 @@ __device__ __forceinline__ void minmod_pair(double b, double c, double d, double
 template <int S>
 __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR[5], double gamma, double inv_gm1,
                                              double F[5]) {
-  // c = sqrt(gamma p / rho) = gamma p * rsqrt(gamma p rho): no division (rsqrt: <= 1 ulp)
+  // c = sqrt(gamma p / rho) = gamma p * rsqrt(gamma p rho): no division
   const double gpL = gamma * WL[4], gpR = gamma * WR[4];
-  const double cL = gpL * rsqrt(gpL * WL[0]);
-  const double cR = gpR * rsqrt(gpR * WR[0]);
+  const double cL = gpL * fast_rsqrt(gpL * WL[0]);
+  const double cR = gpR * fast_rsqrt(gpR * WR[0]);
   const double SL = fmin(WL[1] - cL, WR[1] - cR);
   const double SR = fmax(WL[1] + cL, WR[1] + cR);
-  const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));
-  const double ER = WR[4] * inv_gm1 + 0.5 * WR[0] * (WR[1] * WR[1] + (WR[2] * WR[2] + WR[3] * WR[3]));
-  const double UL[5] = { WL[0], WL[0] * WL[1], WL[0] * WL[2], WL[0] * WL[3], EL };
-  const double UR[5] = { WR[0], WR[0] * WR[1], WR[0] * WR[2], WR[0] * WR[3], ER };
-  const double FL[5] = { UL[1], UL[1] * WL[1] + WL[4], UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
-  const double FR[5] = { UR[1], UR[1] * WR[1] + WR[4], UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
-  if (SL >= 0.0) {
+  if (S == SCHEME_A) {                                   // HLL needs both sides' U and F
+    const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));
+    const double ER = WR[4] * inv_gm1 + 0.5 * WR[0] * (WR[1] * WR[1] + (WR[2] * WR[2] + WR[3] * WR[3]));
+    const double UL[5] = { WL[0], WL[0] * WL[1], WL[0] * WL[2], WL[0] * WL[3], EL };
+    const double UR[5] = { WR[0], WR[0] * WR[1], WR[0] * WR[2], WR[0] * WR[3], ER };
+    const double FL[5] = { UL[1], UL[1] * WL[1] + WL[4], UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
+    const double FR[5] = { UR[1], UR[1] * WR[1] + WR[4], UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
+    if (SL >= 0.0) {
 #pragma unroll
-    for (int m = 0; m < 5; ++m) F[m] = FL[m];
-    return;
-  }
-  if (SR <= 0.0) {
+      for (int m = 0; m < 5; ++m) F[m] = FL[m];
+      return;
+    }
+    if (SR <= 0.0) {
 #pragma unroll
-    for (int m = 0; m < 5; ++m) F[m] = FR[m];
-    return;
-  }
-  if (S == SCHEME_A) {                                   // HLL
+      for (int m = 0; m < 5; ++m) F[m] = FR[m];
+      return;
+    }
     const double inv = fast_rcp(SR - SL);
     const double ss = SL * SR;
 #pragma unroll
     for (int m = 0; m < 5; ++m) F[m] = ((SR * FL[m] - SL * FR[m]) + ss * (UR[m] - UL[m])) * inv;
-  } else {                                               // HLLC, averaged-pressure form (G5)
+  } else {
+    // HLLC, averaged-pressure form (G5).  Only the upwind side's U and F enter the result: side L if
+    // SL >= 0 or (SR > 0 and S* > 0), else side R; the supersonic cases return that side's F.
     const double A = WL[0] * (SL - WL[1]);
     const double B = WR[0] * (SR - WR[1]);
     const double Ss = ((WR[4] - WL[4]) + (A * WL[1] - B * WR[1])) * fast_rcp(A - B);
     const double pbar = 0.5 * ((WL[4] + WR[4]) + (A * (Ss - WL[1]) + B * (Ss - WR[1])));
+    const bool supL = SL >= 0.0, supR = !supL && SR <= 0.0;
+    const bool left = supL || (!supR && Ss > 0.0);
+    double W[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) W[m] = left ? WL[m] : WR[m];
+    const double SK = left ? SL : SR;
+    const double E = W[4] * inv_gm1 + 0.5 * W[0] * (W[1] * W[1] + (W[2] * W[2] + W[3] * W[3]));
+    const double UK[5] = { W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E };
+    const double FK[5] = { UK[1], UK[1] * W[1] + W[4], UK[1] * W[2], UK[1] * W[3], (E + W[4]) * W[1] };
+    if (supL || supR) {
+#pragma unroll
+      for (int m = 0; m < 5; ++m) F[m] = FK[m];
+      return;
+    }
     if (Ss == 0.0) {
       F[0] = 0.0; F[1] = pbar; F[2] = 0.0; F[3] = 0.0; F[4] = 0.0;
       return;
     }
-    const bool left = Ss > 0.0;
-    const double SK = left ? SL : SR;
     const double inv = fast_rcp(SK - Ss);
     const double sp = SK * pbar;
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
-      const double UK = left ? UL[m] : UR[m];
-      const double FK = left ? FL[m] : FR[m];
-      const double D = (m == 1) ? 1.0 : (m == 4) ? Ss : 0.0;
-      F[m] = (Ss * (SK * UK - FK) + sp * D) * inv;
+      double t = Ss * (SK * UK[m] - FK[m]);
+      if (m == 1) t += sp;
+      if (m == 4) t = fma(sp, Ss, t);
+      F[m] = t * inv;
     }
   }
 }
