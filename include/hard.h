@@ -38,7 +38,8 @@ typedef struct hard_ctx hard_ctx; /* opaque, one per simulation */
 
 enum { HARD_OK = 0, HARD_ERR_ARG = -1, HARD_ERR_CUDA = -2, HARD_ERR_NOMEM = -3, HARD_ERR_NOSTATE = -4,
        HARD_ERR_NONPHYSICAL = -5 };
-enum { HARD_BC_PERIODIC = 0, HARD_BC_OUTFLOW = 1 }; /* applied on all faces of active dimensions (G10) */
+enum { HARD_BC_PERIODIC = 0, HARD_BC_OUTFLOW = 1,    /* applied on all faces of active dimensions (G10) */
+       HARD_BC_REFLECT = 2 };                        /* reflecting wall: mirror image, normal momentum negated (G17) */
 enum { HARD_SCHEME_WENO5Z_HLL = 0,   /* the paper's scheme, P:151 (default)                       */
        HARD_SCHEME_MUSCL_HLLC = 1 }; /* BJ fallback: MUSCL-minmod + HLLC                          */
 enum { HARD_VARIANT_FUSED = 0,       /* one kernel per RK stage (BJ "fused RK stage")             */

@@ -22,6 +22,7 @@ SCHEME_A = 0  # WENO5-Z + HLL + Heun (paper)
 SCHEME_B = 1  # MUSCL-minmod + HLLC + SSP-RK2 (north_star fallback)
 BC_PERIODIC = 0
 BC_OUTFLOW = 1
+BC_REFLECT = 2   # reflecting wall (NEXT-2, G17)
 ERR_NONPHYSICAL = -5
 
 # -ffp-contract=off: no FMA contraction, so every operation rounds once in the order written.

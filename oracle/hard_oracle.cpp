@@ -19,7 +19,7 @@
 //                                                                                  (scheme 1, "B")
 //   Heun's method, tableau 0 | 1 1 | 1/2 1/2                      P:151-160 Table 2
 //   dt from the CFL condition                                     P:215, P:255     (formula: G6)
-//   ghost entities of the N-array topology                        P:64             (BCs: G10)
+//   ghost entities of the N-array topology                        P:64             (BCs: G10, G17)
 // Every place where the paper is silent is a DESIGN.md reading (G1..G13) and is marked below.
 //
 // Pins (tests/test_oracle_*.py, all -m "not gpu"): exact Sod / LeBlanc Riemann solutions and L1
@@ -38,7 +38,7 @@
 namespace {
 
 enum { ORC_OK = 0, ORC_ERR_ARG = -1, ORC_ERR_NOSTATE = -4, ORC_ERR_NONPHYSICAL = -5 };
-enum { BC_PERIODIC = 0, BC_OUTFLOW = 1 };
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2 };
 enum { SCHEME_A = 0, SCHEME_B = 1 };
 
 // G8: permutation-symmetric, sign-odd three-term sum.  Order by magnitude, add the two smallest
@@ -205,14 +205,17 @@ void fill_ghosts(const Ctx* c, std::vector<double> V[5]) {
           for (int m = 1; m <= c->g; ++m) {
             ijk[b1] = q1; ijk[b2] = q2;
             int lo_src, hi_src;
-            if (c->bc == BC_PERIODIC) { lo_src = c->n[a] - m; hi_src = m - 1; }
-            else                      { lo_src = 0;           hi_src = c->n[a] - 1; }
+            if (c->bc == BC_PERIODIC)     { lo_src = c->n[a] - m; hi_src = m - 1; }
+            else if (c->bc == BC_REFLECT) { lo_src = m - 1;       hi_src = c->n[a] - m; }   // mirror image (G17)
+            else                          { lo_src = 0;           hi_src = c->n[a] - 1; }
             ijk[a] = lo_src;  long s_lo = c->idx(ijk[0], ijk[1], ijk[2]);
             ijk[a] = -m;      long d_lo = c->idx(ijk[0], ijk[1], ijk[2]);
             ijk[a] = hi_src;  long s_hi = c->idx(ijk[0], ijk[1], ijk[2]);
             ijk[a] = c->n[a] - 1 + m; long d_hi = c->idx(ijk[0], ijk[1], ijk[2]);
-            V[f][d_lo] = V[f][s_lo];
-            V[f][d_hi] = V[f][s_hi];
+            // reflecting wall: the ghost state is the mirror image, i.e. the normal momentum changes sign
+            const double sgn = (c->bc == BC_REFLECT && f == 1 + a) ? -1.0 : 1.0;
+            V[f][d_lo] = sgn * V[f][s_lo];
+            V[f][d_hi] = sgn * V[f][s_hi];
           }
   }
 }
@@ -327,7 +330,7 @@ void step_dt(Ctx* c, double dt) {
 extern "C" {
 
 void* oracle_create(int nx, int ny, int nz, double gamma, int bc) {
-  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != BC_PERIODIC && bc != BC_OUTFLOW)) return nullptr;
+  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != BC_PERIODIC && bc != BC_OUTFLOW && bc != BC_REFLECT)) return nullptr;
   Ctx* c = new Ctx();
   c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
   c->gamma = gamma; c->bc = bc; c->scheme = SCHEME_A;

@@ -317,7 +317,7 @@ extern "C" {
 
 hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc) {
   g_create_error.clear();
-  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != HARD_BC_PERIODIC && bc != HARD_BC_OUTFLOW)) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != HARD_BC_PERIODIC && bc != HARD_BC_OUTFLOW && bc != HARD_BC_REFLECT)) {
     g_create_error = "hard_create: bad argument";
     return nullptr;
   }

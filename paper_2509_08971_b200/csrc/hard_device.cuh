@@ -74,8 +74,9 @@ __device__ __forceinline__ void wenoz_pair(double a, double b, double c, double 
   const double tau = fabs(B0 - B2);
   const double P12 = B1 * B2, P02 = B0 * B2, P01 = B0 * B1;
   const double T0 = B0 + tau, T1 = B1 + tau, T2 = B2 + tau;
-  const double a0 = (0.1 * T0) * P12, a1 = (0.6 * T1) * P02, a2 = (0.3 * T2) * P01;   // plus weights
-  const double m0 = (0.1 * T2) * P01, m2 = (0.3 * T0) * P12;                           // minus (m1 = a1)
+  const double a0 = (0.1 * T0) * P12, a1 = (0.6 * T1) * P02;                // plus weights (unnormalised)
+  const double m0 = (0.1 * T2) * P01;                                       // minus weights; m1 = a1
+  const double a2 = 3.0 * m0, m2 = 3.0 * a0;                                // 0.3 T2 P01 and 0.3 T0 P12
   const double sp = (a0 + a1) + a2, sm = (m0 + a1) + m2;
   // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
   const double q0 = fma(5.0, d2, -2.0 * d1), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);

@@ -22,7 +22,7 @@ struct GridDesc {
   long long pitch, plane, fstride;   // doubles: row, z-plane, field
   double inv_d[3];
   double gamma;
-  int bc;                   // 0 periodic, 1 outflow
+  int bc;                   // 0 periodic, 1 outflow, 2 reflecting
   int g;                    // ghost width of the scheme
 };
 
@@ -95,16 +95,19 @@ __global__ void ghost_fill_kernel(double* __restrict__ U, GridDesc g, DevScalars
     int dst, src;
     if (m < G) {                                    // low side, layer m+1
       dst = -(m + 1);
-      src = (g.bc == 0) ? n - (m + 1) : 0;
+      src = (g.bc == 0) ? n - (m + 1) : (g.bc == 2) ? m : 0;
     } else {                                        // high side, layer m-G+1
       const int l = m - G;
       dst = n + l;
-      src = (g.bc == 0) ? l : n - 1;
+      src = (g.bc == 0) ? l : (g.bc == 2) ? n - 1 - l : n - 1;
     }
     c[d] = dst; const long long pd = cell_addr(g, c[0], c[1], c[2]);
     c[d] = src; const long long ps = cell_addr(g, c[0], c[1], c[2]);
 #pragma unroll
-    for (int f = 0; f < 5; ++f) U[f * g.fstride + pd] = U[f * g.fstride + ps];
+    for (int f = 0; f < 5; ++f) {
+      const double v = U[f * g.fstride + ps];
+      U[f * g.fstride + pd] = (g.bc == 2 && f == 1 + d) ? -v : v;   // reflecting wall: mirror image
+    }
   }
 }
 

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libhard_b200.so")
 
 OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_NOSTATE, ERR_NONPHYSICAL = 0, -1, -2, -3, -4, -5
-BC_PERIODIC, BC_OUTFLOW = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT = 0, 1, 2
 SCHEME_WENO5Z_HLL, SCHEME_MUSCL_HLLC = 0, 1
 VARIANT_FUSED, VARIANT_PERDIR = 0, 1
 

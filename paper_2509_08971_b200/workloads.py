@@ -13,6 +13,7 @@ import numpy as np
 
 BC_PERIODIC = 0
 BC_OUTFLOW = 1
+BC_REFLECT = 2
 _M64 = (1 << 64) - 1
 
 
@@ -160,6 +161,26 @@ def turbulence(n=512, nsteps=20, cfl=0.4, seed=12345, device=None, slab=64):
             del ke, v
     return Workload("turb%d" % n, (n, n, n), g, BC_PERIODIC, (d, d, d), cfl, nsteps=nsteps, state=st,
                     meta={"seed": seed, "modes": modes})
+
+
+def kelvin_helmholtz(n=256, t_end=None, nsteps=100, cfl=0.4, gamma=1.4, p0=2.5, amp=0.01):
+    """NEXT-2: non-radiative panel of the paper's 2-D Kelvin-Helmholtz run:
+    [-0.5,0.5]^2, rho_low = 1, rho_high = 2.5 in the layer |y| <= 0.25, v_x = -0.5 in the layer and +0.5
+    elsewhere.  The paper gives neither pressure, gamma, grid, boundaries nor the seed perturbation
+    (G18): p = 2.5, gamma = 1.4, periodic, n x n x 1, v_y = amp sin(4 pi x) (exp(-(y-1/4)^2/s^2)
+    + exp(-(y+1/4)^2/s^2)), s = 0.05."""
+    d = 1.0 / n
+    xc = -0.5 + (np.arange(n) + 0.5) * d
+    Y, X = np.meshgrid(xc, xc, indexing="ij")
+    layer = np.abs(Y) <= 0.25
+    rho = np.where(layer, 2.5, 1.0)
+    u = np.where(layer, -0.5, 0.5)
+    s2 = 0.05 ** 2
+    v = amp * np.sin(4.0 * np.pi * X) * (np.exp(-(Y - 0.25) ** 2 / s2) + np.exp(-(Y + 0.25) ** 2 / s2))
+    p = np.full_like(rho, p0)
+    z = np.zeros_like(rho)
+    st = [a.reshape(1, n, n) for a in _cons(rho, u, v, z, p, gamma)]
+    return Workload("kh%d" % n, (n, n, 1), gamma, BC_PERIODIC, (d, d, 1.0), cfl, t_end=t_end, nsteps=nsteps, state=st)
 
 
 def random_state(n, seed, gamma=1.4, amp=0.3):

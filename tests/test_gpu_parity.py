@@ -118,3 +118,20 @@ def test_device_pointers_and_uniform_state():
         for a, b in zip(out, st):
             assert torch.equal(a, b)        # uniform state preserved exactly
         h.close()
+
+
+# ---------------------------------------------------------------- NEXT-2: reflecting walls, Kelvin-Helmholtz
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("n", [(37, 21, 19), (45, 30, 1), (131, 1, 1)])
+def test_reflecting_walls(scheme, variant, n):
+    w = _random_workload(n, wl.BC_REFLECT, seed=7 + sum(n), spacing=(0.1, 0.07, 0.13))
+    _check(w, scheme, variant, 1, TOL_1)
+    _check(w, scheme, variant, 25, TOL_100)
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_kelvin_helmholtz_2d(scheme):
+    w = wl.kelvin_helmholtz(256, nsteps=100)
+    _check(w, scheme, hard.VARIANT_FUSED, 1, TOL_1)
+    _check(w, scheme, hard.VARIANT_FUSED, 100, TOL_100)
