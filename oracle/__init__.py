@@ -71,6 +71,11 @@ def lib():
         L.oracle_cons_to_prim.argtypes = [dp, ctypes.c_double, dp]
         L.oracle_riemann.restype = None
         L.oracle_riemann.argtypes = [ctypes.c_int, dp, dp, ctypes.c_int, ctypes.c_double, dp]
+        L.oracle_enable_radiation.argtypes = [vp]
+        L.oracle_set_rad_energy.argtypes = [vp, dp]
+        L.oracle_get_rad_energy.argtypes = [vp, dp]
+        L.oracle_rusanov.restype = ctypes.c_double
+        L.oracle_rusanov.argtypes = [ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_double]
         _lib = L
     return _lib
 
@@ -92,7 +97,7 @@ class Oracle:
     (rho, mx, my, mz, E) of P:93 eq.2.
     """
 
-    def __init__(self, nx, ny, nz, gamma, bc, scheme=SCHEME_A, spacing=None, check=True):
+    def __init__(self, nx, ny, nz, gamma, bc, scheme=SCHEME_A, spacing=None, check=True, radiation=False):
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.h = self.L.oracle_create(nx, ny, nz, gamma, bc)
@@ -101,6 +106,8 @@ class Oracle:
         self._chk(self.L.oracle_set_scheme(self.h, scheme), "set_scheme")
         if spacing is not None:
             self._chk(self.L.oracle_set_spacing(self.h, *map(float, spacing)), "set_spacing")
+        if radiation:
+            self._chk(self.L.oracle_enable_radiation(self.h), "enable_radiation")
         if not check:
             self._chk(self.L.oracle_set_check(self.h, 0), "set_check")
 
@@ -126,6 +133,15 @@ class Oracle:
     def get_state(self):
         out = [np.empty(self.shape, dtype=np.float64) for _ in range(5)]
         self._chk(self.L.oracle_get_state(self.h, *[_dp(a) for a in out]), "get_state")
+        return out
+
+    def set_rad_energy(self, er):
+        a = np.ascontiguousarray(er, dtype=np.float64).reshape(self.shape)
+        self._chk(self.L.oracle_set_rad_energy(self.h, _dp(a)), "set_rad_energy")
+
+    def get_rad_energy(self):
+        out = np.empty(self.shape, dtype=np.float64)
+        self._chk(self.L.oracle_get_rad_energy(self.h, _dp(out)), "get_rad_energy")
         return out
 
     def step(self, cfl, nsteps=1):
@@ -190,3 +206,9 @@ def riemann(scheme, WL, WR, direction, gamma):
     F = np.empty(5)
     lib().oracle_riemann(int(scheme), _dp(WL), _dp(WR), int(direction), float(gamma), _dp(F))
     return F
+
+
+def rusanov(EL, ER, WL, WR, direction, gamma):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    return lib().oracle_rusanov(float(EL), float(ER), _dp(WL), _dp(WR), int(direction), float(gamma))

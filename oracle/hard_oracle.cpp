@@ -20,6 +20,8 @@
 //   Heun's method, tableau 0 | 1 1 | 1/2 1/2                      P:151-160 Table 2
 //   dt from the CFL condition                                     P:215, P:255     (formula: G6)
 //   ghost entities of the N-array topology                        P:64             (BCs: G10, G17)
+//   radiation energy density advected with the fluid, Rusanov    P:93 eq.2 (4th row), eq.14 LHS,
+//   (local Lax-Friedrichs) flux                                   P:151            (NEXT-1; G19)
 // Every place where the paper is silent is a DESIGN.md reading (G1..G13) and is marked below.
 //
 // Pins (tests/test_oracle_*.py, all -m "not gpu"): exact Sod / LeBlanc Riemann solutions and L1
@@ -29,6 +31,7 @@
 // candidate stencils, flux consistency F*(W,W) = F(W), stationary contact under HLLC, and a
 // hand-unrolled brute-force step on a 4x4x4 periodic grid.  No function here is "parity unpinned".
 
+#include <algorithm>
 #include <cmath>
 #include <cstddef>
 #include <cstdlib>
@@ -53,7 +56,7 @@ double sum3sym(double a, double b, double c) {
 }
 
 struct Prim { double rho, v[3], p; };          // primitive state (rho, u, v, w, p)        G3
-struct Cons { double q[5]; };                  // (rho, mx, my, mz, E)
+struct Cons { double q[6]; };                  // (rho, mx, my, mz, E [, E_rad])
 
 // a2: conserved -> primitive with the ideal-gas EOS.
 Prim cons_to_prim(const double U[5], double gamma) {
@@ -163,6 +166,16 @@ void riemann(int scheme, const Prim& WL, const Prim& WR, int dir, double gamma, 
   F[4] = Fl[4];
 }
 
+// NEXT-1 (G19): local Lax-Friedrichs (Rusanov) flux of the advected radiation energy density
+// (advection part of P:141 eq.14: d_t E + d_j(E v^j) = 0).  EL/ER and the primitive states are
+// the reconstructed face values; alpha = max(|u_n| + c_s) over the two sides.
+double rusanov(double EL, double ER, const Prim& WL, const Prim& WR, int dir, double gamma) {
+  double unL = WL.v[dir], unR = WR.v[dir];
+  double cL = std::sqrt(gamma * WL.p / WL.rho), cR = std::sqrt(gamma * WR.p / WR.rho);
+  double alpha = std::fmax(std::fabs(unL) + cL, std::fabs(unR) + cR);
+  return 0.5 * (EL * unL + ER * unR) - 0.5 * alpha * (ER - EL);
+}
+
 struct Ctx {
   int n[3];                 // interior cells per direction
   int gh[3];                // ghost width per direction (g if n>1, else 0: G11)
@@ -170,7 +183,8 @@ struct Ctx {
   int g;                    // 3 for scheme A, 2 for scheme B
   int scheme, bc;
   double gamma, d[3];
-  std::vector<double> U[5], U1[5];
+  int nf;                   // 5, or 6 with the advected radiation energy density (NEXT-1)
+  std::vector<double> U[6], U1[6];
   double lambda, t;
   long long steps;
   long long fallbacks;      // G4 positivity fallbacks taken so far
@@ -189,17 +203,17 @@ void layout(Ctx* c) {
     c->P[a] = c->n[a] + 2 * c->gh[a];
   }
   size_t tot = (size_t)c->P[0] * c->P[1] * c->P[2];
-  for (int f = 0; f < 5; ++f) { c->U[f].assign(tot, 0.0); c->U1[f].assign(tot, 0.0); }
+  for (int f = 0; f < 6; ++f) { c->U[f].assign(f < c->nf ? tot : 0, 0.0); c->U1[f].assign(f < c->nf ? tot : 0, 0.0); }
   c->have_state = 0;
 }
 
 // a1: ghost-cell fill (P:64 ghost entities; G10).  Faces only: the stencils are one-dimensional.
-void fill_ghosts(const Ctx* c, std::vector<double> V[5]) {
+void fill_ghosts(const Ctx* c, std::vector<double> V[6]) {
   for (int a = 0; a < 3; ++a) {
     if (!c->active(a)) continue;
     const int b1 = (a + 1) % 3, b2 = (a + 2) % 3;
     int ijk[3];
-    for (int f = 0; f < 5; ++f)
+    for (int f = 0; f < c->nf; ++f)
       for (int q2 = 0; q2 < c->n[b2]; ++q2)
         for (int q1 = 0; q1 < c->n[b1]; ++q1)
           for (int m = 1; m <= c->g; ++m) {
@@ -221,7 +235,7 @@ void fill_ghosts(const Ctx* c, std::vector<double> V[5]) {
 }
 
 // a7: max wavespeed over interior cells (G6).  Returns lambda; flags non-physical cells.
-double maxwavespeed(Ctx* c, const std::vector<double> V[5]) {
+double maxwavespeed(Ctx* c, const std::vector<double> V[6]) {
   double lam = 0.0;
   for (int k = 0; k < c->n[2]; ++k)
     for (int j = 0; j < c->n[1]; ++j)
@@ -242,17 +256,19 @@ double maxwavespeed(Ctx* c, const std::vector<double> V[5]) {
 
 // L(U) (eq.15): dF[a][f][cell] = (F*_{+1/2} - F*_{-1/2}) / Delta_a, per direction, then
 // L = -sum3sym over directions.  Lout[f] is indexed over interior cells i + nx (j + ny k).
-void rhs(Ctx* c, const std::vector<double> V[5], std::vector<double> Lout[5]) {
+void rhs(Ctx* c, const std::vector<double> V[6], std::vector<double> Lout[6]) {
   const long N = c->ncell();
-  std::vector<double> dF[3][5];
+  const int nf = c->nf;
+  std::vector<double> dF[3][6];
   for (int a = 0; a < 3; ++a)
-    for (int f = 0; f < 5; ++f) dF[a][f].assign(N, 0.0);
+    for (int f = 0; f < nf; ++f) dF[a][f].assign(N, 0.0);
   const int r = c->g - 1;                                    // reconstruction stencil radius
   for (int a = 0; a < 3; ++a) {
     if (!c->active(a)) continue;
     const int b1 = (a + 1) % 3, b2 = (a + 2) % 3;
     const int na = c->n[a], g = c->g;
     std::vector<Prim> W(na + 2 * g), Wp(na + 2 * g), Wm(na + 2 * g);   // index s = i + g
+    std::vector<double> Er(na + 2 * g), Erp(na + 2 * g), Erm(na + 2 * g);  // radiation energy density (nf = 6)
     std::vector<Cons> Fs(na + 1);                                      // face i+1/2 at slot i+1
     int ijk[3];
     for (int q2 = 0; q2 < c->n[b2]; ++q2)
@@ -263,6 +279,7 @@ void rhs(Ctx* c, const std::vector<double> V[5], std::vector<double> Lout[5]) {
           long p = c->idx(ijk[0], ijk[1], ijk[2]);
           double u5[5] = { V[0][p], V[1][p], V[2][p], V[3][p], V[4][p] };
           W[i + g] = cons_to_prim(u5, c->gamma);
+          if (nf == 6) Er[i + g] = V[5][p];
         }
         for (int i = -1; i <= na; ++i) {                               // a3
           double w[5], pl[5], mi[5];
@@ -275,26 +292,35 @@ void rhs(Ctx* c, const std::vector<double> V[5], std::vector<double> Lout[5]) {
             }
             reconstruct(c->scheme, w, &pl[v], &mi[v]);
           }
+          double epl = 0.0, emi = 0.0;
+          if (nf == 6) {                                               // "WENO5-Z for all variables"
+            for (int s = -2; s <= 2; ++s) w[s + 2] = (s < -r || s > r) ? 0.0 : Er[i + s + g];
+            reconstruct(c->scheme, w, &epl, &emi);
+          }
           if (c->scheme == SCHEME_A && (pl[0] <= 0.0 || pl[4] <= 0.0 || mi[0] <= 0.0 || mi[4] <= 0.0)) {
             const Prim& q = W[i + g];                                  // G4: piecewise constant
             pl[0] = mi[0] = q.rho; pl[4] = mi[4] = q.p;
             for (int m = 0; m < 3; ++m) pl[1 + m] = mi[1 + m] = q.v[m];
+            if (nf == 6) epl = emi = Er[i + g];                        // G19: the fallback takes E_rad along
             c->fallbacks++;
           }
+          Erp[i + g] = epl; Erm[i + g] = emi;
           Prim& P = Wp[i + g]; Prim& M = Wm[i + g];
           P.rho = pl[0]; P.p = pl[4]; M.rho = mi[0]; M.p = mi[4];
           for (int m = 0; m < 3; ++m) { P.v[m] = pl[1 + m]; M.v[m] = mi[1 + m]; }
         }
-        for (int i = -1; i < na; ++i)                                  // a4: face between i, i+1
+        for (int i = -1; i < na; ++i) {                                // a4: face between i, i+1
           riemann(c->scheme, Wp[i + g], Wm[i + 1 + g], a, c->gamma, Fs[i + 1].q);
+          if (nf == 6) Fs[i + 1].q[5] = rusanov(Erp[i + g], Erm[i + 1 + g], Wp[i + g], Wm[i + 1 + g], a, c->gamma);
+        }
         for (int i = 0; i < na; ++i) {                                 // a5
           ijk[a] = i;
           long cell = (long)ijk[0] + (long)c->n[0] * ((long)ijk[1] + (long)c->n[1] * ijk[2]);
-          for (int f = 0; f < 5; ++f) dF[a][f][cell] = (Fs[i + 1].q[f] - Fs[i].q[f]) / c->d[a];
+          for (int f = 0; f < nf; ++f) dF[a][f][cell] = (Fs[i + 1].q[f] - Fs[i].q[f]) / c->d[a];
         }
       }
   }
-  for (int f = 0; f < 5; ++f) {
+  for (int f = 0; f < nf; ++f) {
     Lout[f].resize(N);
     for (long p = 0; p < N; ++p) Lout[f][p] = -sum3sym(dF[0][f][p], dF[1][f][p], dF[2][f][p]);
   }
@@ -302,14 +328,14 @@ void rhs(Ctx* c, const std::vector<double> V[5], std::vector<double> Lout[5]) {
 
 // One Heun / SSP-RK2 step with a given dt (Table 2; Shu-Osher form, G7).
 void step_dt(Ctx* c, double dt) {
-  std::vector<double> L[5];
+  std::vector<double> L[6];
   fill_ghosts(c, c->U);
   rhs(c, c->U, L);
   for (int k = 0; k < c->n[2]; ++k)
     for (int j = 0; j < c->n[1]; ++j)
       for (int i = 0; i < c->n[0]; ++i) {
         long p = c->idx(i, j, k), q = (long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k);
-        for (int f = 0; f < 5; ++f) c->U1[f][p] = c->U[f][p] + dt * L[f][q];
+        for (int f = 0; f < c->nf; ++f) c->U1[f][p] = c->U[f][p] + dt * L[f][q];
       }
   fill_ghosts(c, c->U1);
   rhs(c, c->U1, L);
@@ -317,7 +343,7 @@ void step_dt(Ctx* c, double dt) {
     for (int j = 0; j < c->n[1]; ++j)
       for (int i = 0; i < c->n[0]; ++i) {
         long p = c->idx(i, j, k), q = (long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k);
-        for (int f = 0; f < 5; ++f)
+        for (int f = 0; f < c->nf; ++f)
           c->U[f][p] = 0.5 * c->U[f][p] + 0.5 * (c->U1[f][p] + dt * L[f][q]);
       }
   if (c->check) c->lambda = maxwavespeed(c, c->U);
@@ -333,7 +359,7 @@ void* oracle_create(int nx, int ny, int nz, double gamma, int bc) {
   if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != BC_PERIODIC && bc != BC_OUTFLOW && bc != BC_REFLECT)) return nullptr;
   Ctx* c = new Ctx();
   c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
-  c->gamma = gamma; c->bc = bc; c->scheme = SCHEME_A;
+  c->gamma = gamma; c->bc = bc; c->scheme = SCHEME_A; c->nf = 5;
   c->d[0] = 1.0 / nx; c->d[1] = 1.0 / ny; c->d[2] = 1.0 / nz;
   c->lambda = 0.0; c->t = 0.0; c->steps = 0; c->fallbacks = 0;
   c->status = ORC_OK; c->check = 1;
@@ -350,6 +376,38 @@ int oracle_set_spacing(void* h, double dx, double dy, double dz) {
   c->d[0] = dx; c->d[1] = dy; c->d[2] = dz;
   if (c->have_state && c->check) c->lambda = maxwavespeed(c, c->U);
   return ORC_OK;
+}
+
+// NEXT-1: switch the advected radiation energy density on (6 fields); only before oracle_set_state.
+int oracle_enable_radiation(void* h) {
+  Ctx* c = (Ctx*)h;
+  if (!c || c->have_state) return ORC_ERR_ARG;
+  c->nf = 6;
+  layout(c);
+  return ORC_OK;
+}
+
+// Interior copy of E_rad, layout as the other fields; after oracle_set_state (which zeroes E_rad).
+int oracle_set_rad_energy(void* h, const double* er) {
+  Ctx* c = (Ctx*)h;
+  if (!c || !er || c->nf != 6) return ORC_ERR_ARG;
+  if (!c->have_state) return ORC_ERR_NOSTATE;
+  for (int k = 0; k < c->n[2]; ++k)
+    for (int j = 0; j < c->n[1]; ++j)
+      for (int i = 0; i < c->n[0]; ++i)
+        c->U[5][c->idx(i, j, k)] = er[(long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k)];
+  return ORC_OK;
+}
+
+int oracle_get_rad_energy(void* h, double* er) {
+  Ctx* c = (Ctx*)h;
+  if (!c || !er || c->nf != 6) return ORC_ERR_ARG;
+  if (!c->have_state) return ORC_ERR_NOSTATE;
+  for (int k = 0; k < c->n[2]; ++k)
+    for (int j = 0; j < c->n[1]; ++j)
+      for (int i = 0; i < c->n[0]; ++i)
+        er[(long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k)] = c->U[5][c->idx(i, j, k)];
+  return c->status;
 }
 
 int oracle_set_scheme(void* h, int scheme) {
@@ -379,6 +437,7 @@ int oracle_set_state(void* h, const double* rho, const double* mx, const double*
       for (int j = 0; j < c->n[1]; ++j)
         for (int i = 0; i < c->n[0]; ++i)
           c->U[f][c->idx(i, j, k)] = src[f][(long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k)];
+  if (c->nf == 6) std::fill(c->U[5].begin(), c->U[5].end(), 0.0);
   c->have_state = 1;
   c->status = ORC_OK;
   c->t = 0.0; c->steps = 0; c->fallbacks = 0;
@@ -453,6 +512,14 @@ void oracle_riemann(int scheme, const double WL[5], const double WR[5], int dir,
   L.rho = WL[0]; L.v[0] = WL[1]; L.v[1] = WL[2]; L.v[2] = WL[3]; L.p = WL[4];
   R.rho = WR[0]; R.v[0] = WR[1]; R.v[1] = WR[2]; R.v[2] = WR[3]; R.p = WR[4];
   riemann(scheme, L, R, dir, gamma, F);
+}
+
+// NEXT-1: WL, WR = (rho, u, v, w, p) face states; returns the Rusanov flux of E_rad.
+double oracle_rusanov(double EL, double ER, const double WL[5], const double WR[5], int dir, double gamma) {
+  Prim L, R;
+  L.rho = WL[0]; L.v[0] = WL[1]; L.v[1] = WL[2]; L.v[2] = WL[3]; L.p = WL[4];
+  R.rho = WR[0]; R.v[0] = WR[1]; R.v[1] = WR[2]; R.v[2] = WR[3]; R.p = WR[4];
+  return rusanov(EL, ER, L, R, dir, gamma);
 }
 
 }  // extern "C"
