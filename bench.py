@@ -48,6 +48,7 @@ def parse():
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--scheme", default="A", choices=["A", "B"])
     ap.add_argument("--variant", default="fused", choices=["fused", "perdir"])
+    ap.add_argument("--radiation", action="store_true", help="NEXT-1: carry E_rad as a sixth advected field")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -177,8 +178,11 @@ def run_cuda(args):
     variant = hard.VARIANT_FUSED if args.variant == "fused" else hard.VARIANT_PERDIR
     w = wl.turbulence(n, nsteps=K, device=dev)
     cells = n ** 3
-    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing, radiation=args.radiation)
     stream = torch.cuda.current_stream()
+    nfields = 6 if args.radiation else 5
+    alg_bytes = ALG_BYTES_PER_CELL_STAGE * nfields / 5.0
+    e_rad = (1.0 + 0.3 * w.state[0]) if args.radiation else None      # seeded, positive, non-uniform
 
     def barrier():
         if world > 1:
@@ -187,8 +191,12 @@ def run_cuda(args):
 
     # ---- device-resident timing: inputs already in HBM when the timed region starts
     h.set_state(*w.state)
+    if args.radiation:
+        h.set_rad_energy(e_rad)
     h.step(w.cfl, W)                       # warm-up steps (untimed)
     h.set_state(*w.state)                  # timed steps are exactly the workload's steps 1..K
+    if args.radiation:
+        h.set_rad_energy(e_rad)
     fp64_peak = hard.probe_fp64_peak()
     sampler = ClockSampler(local)
     sampler.start()
@@ -224,7 +232,7 @@ def run_cuda(args):
         cell_stages_per_launch = cells                       # one launch = one RK stage over the mesh
     else:
         cell_stages_per_launch = cells * 2.0 * K / max(stage_launches, 1)
-    alg_gbs = cell_stages_per_launch * ALG_BYTES_PER_CELL_STAGE / (per_launch_ms * 1e-3) / 1e9
+    alg_gbs = cell_stages_per_launch * alg_bytes / (per_launch_ms * 1e-3) / 1e9
     alg_tflops = cell_stages_per_launch * ALG_FLOP_PER_CELL_STAGE[args.scheme] / (per_launch_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "stage_kernel<%s>" % args.scheme, "achieved": alg_tflops, "peak": fp64_peak,
                 "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None,
@@ -235,11 +243,11 @@ def run_cuda(args):
                 "alg_flop_per_cell_stage": ALG_FLOP_PER_CELL_STAGE[args.scheme]}
     roofline_hbm = {"bound": "hbm", "achieved": alg_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": alg_gbs / hbm_peak,
                     "frac_of_nominal_8TBs": alg_gbs / 8000.0, "peak_source": hbm_src,
-                    "alg_bytes_per_cell_stage": ALG_BYTES_PER_CELL_STAGE}
+                    "alg_bytes_per_cell_stage": alg_bytes}
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): H2D + K steps + D2H inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.radiation:
         try:
             host_in = [torch.empty((n, n, n), dtype=torch.float64, pin_memory=True) for _ in range(5)]
             for a, b in zip(host_in, w.state):
@@ -278,7 +286,7 @@ def run_cuda(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": "%s: %d^3 periodic seeded sine-mode field, CFL %.2g, %d Heun steps" % (args.workload, n, w.cfl, K),
                            "scheme": "A: WENO5-Z + HLL + Heun (PAPER.md P:151)" if args.scheme == "A" else "B: MUSCL-minmod + HLLC + SSP-RK2 (north_star fallback)",
-                           "variant": args.variant, "parallelism": "replicas x%d" % world,
+                           "variant": args.variant, "fields": nfields, "parallelism": "replicas x%d" % world,
                            "l2": "state (%.1f GB per buffer) is far larger than the 126 MB L2; no flush needed" % (5 * cells * 8 / 1e9),
                            "sim_time": t_sim, "steps_done": steps_done},
                 "roofline": roofline, "roofline_hbm": roofline_hbm, "e2e": e2e, "cpu_baseline": cpu_baseline,

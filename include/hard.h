@@ -79,6 +79,17 @@ int hard_set_spacing(hard_ctx*, double dx, double dy, double dz);
  * before hard_bind_workspace. */
 int hard_set_scheme(hard_ctx*, int scheme);
 
+/* NEXT-1: carry the radiation energy density E_rad as a sixth advected field,
+ * d_t E_rad + d_j(E_rad v^j) = 0 (eq.2 fourth row; advection part of P:141 eq.14), reconstructed like the
+ * other variables, local Lax-Friedrichs (Rusanov) flux with alpha = max(|u_n| + c_s) (G19).  Sources and
+ * diffusion stay out of scope.  Only before hard_set_state / hard_bind_workspace (the layout grows to six fields). */
+int hard_enable_radiation(hard_ctx*);
+
+/* Copy E_rad in / out (host or device pointer, nx*ny*nz doubles, same layout as the other fields).
+ * hard_set_state zeroes E_rad; call hard_set_rad_energy after it.  hard_get_rad_energy synchronises. */
+int hard_set_rad_energy(hard_ctx*, const double* e_rad);
+int hard_get_rad_energy(hard_ctx*, double* e_rad);
+
 /* HARD_VARIANT_*; may be switched at any time between steps (same state buffers). */
 int hard_set_variant(hard_ctx*, int variant);
 

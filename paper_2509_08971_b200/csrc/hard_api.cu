@@ -31,6 +31,7 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct hard_ctx {
   GridDesc g;
   int scheme = HARD_SCHEME_WENO5Z_HLL, variant = HARD_VARIANT_FUSED;
+  int nf = 5;                       // 6 with the advected radiation energy density (hard_enable_radiation)
   cudaStream_t stream = 0;
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -78,6 +79,7 @@ int after_launch(hard_ctx* c, const char* name) {
 void compute_layout(hard_ctx* c) {
   GridDesc& g = c->g;
   g.g = (c->scheme == HARD_SCHEME_WENO5Z_HLL) ? 3 : 2;
+  g.nf = c->nf;
   for (int a = 0; a < 3; ++a) g.act[a] = g.n[a] > 1;
   // x: ghost width g on the left, so that a tile's TMA box (which starts g cells left of the tile)
   // starts at padded x-coordinate i0, a multiple of 16 doubles: the box start must be 16-byte
@@ -95,7 +97,7 @@ void compute_layout(hard_ctx* c) {
   g.fstride = (long long)align_up((size_t)(g.plane * g.P[2]), 32);
 }
 
-size_t state_bytes(const hard_ctx* c) { return (size_t)5 * c->g.fstride * sizeof(double); }
+size_t state_bytes(const hard_ctx* c) { return (size_t)c->nf * c->g.fstride * sizeof(double); }
 
 void carve(hard_ctx* c) {
   char* p = (char*)c->ws;
@@ -119,9 +121,9 @@ int make_map(hard_ctx* c, CUtensorMap* m, double* base) {
   }
   const GridDesc& g = c->g;
   const int BXh = 14 + 2 * g.g, BYh = 16 + 2 * g.g;          // StageCfg<S>::BX, BY
-  cuuint64_t dims[4] = { (cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], 5 };
+  cuuint64_t dims[4] = { (cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], (cuuint64_t)g.nf };
   cuuint64_t strides[3] = { (cuuint64_t)g.pitch * 8, (cuuint64_t)g.plane * 8, (cuuint64_t)g.fstride * 8 };
-  cuuint32_t box[4] = { (cuuint32_t)BXh, (cuuint32_t)BYh, 1, 5 };
+  cuuint32_t box[4] = { (cuuint32_t)BXh, (cuuint32_t)BYh, 1, (cuuint32_t)g.nf };
   cuuint32_t es[4] = { 1, 1, 1, 1 };
   CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -146,12 +148,13 @@ int choose_Lz(const hard_ctx* c) {
   // waves = CTAs / (2 CTAs per SM * SMs) and the +1 is the measured tail of unequal CTA progress
   // (512^3: one 512-plane chunk per tile = exactly 4 waves ran 15 % slower than 64-plane chunks).
   const double lead = 2.0 + 0.5 * (2 * (g.g - 1) + 1);      // z-only iterations + prologue loads, in plane units
+  const double ctas_per_sm = (c->nf == 6 && c->scheme == HARD_SCHEME_WENO5Z_HLL) ? 1.0 : 2.0;
   double best = 1e300;
   int bestc = 1;
   for (int ch = 1; ch <= (nz + 15) / 16; ++ch) {
     const int lz = (nz + ch - 1) / ch;
     const long long ctas = tiles * ((nz + lz - 1) / lz);
-    const double waves = (double)ctas / (2.0 * c->sm_count);
+    const double waves = (double)ctas / (ctas_per_sm * c->sm_count);
     const double cost = (waves + 1.0) * (lz + lead);
     if (cost < best * 0.999) { best = cost; bestc = ch; }
   }
@@ -173,8 +176,10 @@ int ensure_ready(hard_ctx* c) {
     if (rc) return rc;
     rc = make_map(c, &c->tmU1, c->U1);
     if (rc) return rc;
-    CK(cudaFuncSetAttribute(stage_kernel<SCHEME_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<SCHEME_A>::SMEM));
-    CK(cudaFuncSetAttribute(stage_kernel<SCHEME_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<SCHEME_B>::SMEM));
+#define HARD_SET_SMEM(S, NF) \
+  CK(cudaFuncSetAttribute(stage_kernel<S, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM));
+    HARD_SET_SMEM(SCHEME_A, 5) HARD_SET_SMEM(SCHEME_B, 5) HARD_SET_SMEM(SCHEME_A, 6) HARD_SET_SMEM(SCHEME_B, 6)
+#undef HARD_SET_SMEM
     c->Lz = choose_Lz(c);
     c->maps_ready = true;
   }
@@ -235,10 +240,11 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
   dim3 grid((g.n[0] + 13) / 14, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
   int rc = prof_begin(c);
   if (rc) return rc;
-  if (c->scheme == HARD_SCHEME_WENO5Z_HLL)
-    stage_kernel<SCHEME_A><<<grid, 256, StageCfg<SCHEME_A>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
-  else
-    stage_kernel<SCHEME_B><<<grid, 256, StageCfg<SCHEME_B>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a);
+#define HARD_LAUNCH(S, NF) \
+  stage_kernel<S, NF><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a)
+  if (c->scheme == HARD_SCHEME_WENO5Z_HLL) { if (c->nf == 6) HARD_LAUNCH(SCHEME_A, 6); else HARD_LAUNCH(SCHEME_A, 5); }
+  else                                     { if (c->nf == 6) HARD_LAUNCH(SCHEME_B, 6); else HARD_LAUNCH(SCHEME_B, 5); }
+#undef HARD_LAUNCH
   if ((rc = after_launch(c, "stage_kernel"))) return rc;
   return prof_end(c);
 }
@@ -384,6 +390,31 @@ int hard_set_scheme(hard_ctx* c, int scheme) {
   return HARD_OK;
 }
 
+int hard_enable_radiation(hard_ctx* c) {
+  if (!c) return HARD_ERR_ARG;
+  if (c->have_state || c->ws) return fail(c, HARD_ERR_ARG, "hard_enable_radiation: only before hard_set_state / hard_bind_workspace");
+  c->nf = 6;
+  compute_layout(c);
+  return HARD_OK;
+}
+
+int hard_set_rad_energy(hard_ctx* c, const double* er) {
+  if (!c || !er) return fail(c, HARD_ERR_ARG, "hard_set_rad_energy: null pointer");
+  if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_set_rad_energy: call hard_enable_radiation first");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
+  return copy_field(c, c->U + 5 * c->g.fstride, er, true);
+}
+
+int hard_get_rad_energy(hard_ctx* c, double* er) {
+  if (!c || !er) return fail(c, HARD_ERR_ARG, "hard_get_rad_energy: null pointer");
+  if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_get_rad_energy: call hard_enable_radiation first");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
+  int rc = copy_field(c, c->U + 5 * c->g.fstride, er, false);
+  if (rc) return rc;
+  DevScalars h;
+  return sync_status(c, &h);
+}
+
 int hard_set_variant(hard_ctx* c, int variant) {
   if (!c || (variant != HARD_VARIANT_FUSED && variant != HARD_VARIANT_PERDIR))
     return fail(c, HARD_ERR_ARG, "hard_set_variant: unknown variant");
@@ -425,6 +456,7 @@ int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const doubl
   const double* src[5] = { rho, mx, my, mz, E };
   for (int f = 0; f < 5; ++f)
     if ((rc = copy_field(c, c->U + f * c->g.fstride, src[f], true))) return rc;
+  if (c->nf == 6) CK(cudaMemsetAsync(c->U + 5 * c->g.fstride, 0, (size_t)c->g.fstride * sizeof(double), c->stream));
   CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
   c->steps_enq = 0;
   c->have_state = true;

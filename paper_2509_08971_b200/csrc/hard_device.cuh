@@ -103,16 +103,18 @@ __device__ __forceinline__ void minmod_pair(double b, double c, double d, double
 }
 
 // a4 (G2 Davis bounds; G5 inclusive tie-breaks).  WL/WR = (rho, un, ut1, ut2, p) already
-// rotated so that component 1 is the face normal.  F in the same rotated (rho, n, t1, t2, E) order.
+// rotated so that component 1 is the face normal.  F in the same rotated (rho, n, t1, t2, E) order;
+// alpha returns the largest signal speed max(|u_n| + c_s) of the two sides.
 template <int S>
 __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR[5], double gamma, double inv_gm1,
-                                             double F[5]) {
+                                             double F[5], double& alpha) {
   // c = sqrt(gamma p / rho) = gamma p * rsqrt(gamma p rho): no division
   const double gpL = gamma * WL[4], gpR = gamma * WR[4];
   const double cL = gpL * fast_rsqrt(gpL * WL[0]);
   const double cR = gpR * fast_rsqrt(gpR * WR[0]);
   const double SL = fmin(WL[1] - cL, WR[1] - cR);
   const double SR = fmax(WL[1] + cL, WR[1] + cR);
+  alpha = fmax(SR, -SL);                                 // = max(|u_n| + c_s) over the two sides (Rusanov, NEXT-1)
   if (S == SCHEME_A) {                                   // HLL needs both sides' U and F
     const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));
     const double ER = WR[4] * inv_gm1 + 0.5 * WR[0] * (WR[1] * WR[1] + (WR[2] * WR[2] + WR[3] * WR[3]));

@@ -24,6 +24,7 @@ struct GridDesc {
   double gamma;
   int bc;                   // 0 periodic, 1 outflow, 2 reflecting
   int g;                    // ghost width of the scheme
+  int nf;                   // fields per state: 5, or 6 with the advected radiation energy density (NEXT-1)
 };
 
 // Device-resident scalars: nothing returns to the host inside hard_step.
@@ -103,8 +104,7 @@ __global__ void ghost_fill_kernel(double* __restrict__ U, GridDesc g, DevScalars
     }
     c[d] = dst; const long long pd = cell_addr(g, c[0], c[1], c[2]);
     c[d] = src; const long long ps = cell_addr(g, c[0], c[1], c[2]);
-#pragma unroll
-    for (int f = 0; f < 5; ++f) {
+    for (int f = 0; f < g.nf; ++f) {
       const double v = U[f * g.fstride + ps];
       U[f * g.fstride + pd] = (g.bc == 2 && f == 1 + d) ? -v : v;   // reflecting wall: mirror image
     }
@@ -181,8 +181,7 @@ __global__ void axpy_kernel(const double* __restrict__ Un, const double* __restr
     const long long r = idx / g.n[0];
     const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
     const long long p = cell_addr(g, i, j, k);
-#pragma unroll
-    for (int f = 0; f < 5; ++f) {
+    for (int f = 0; f < g.nf; ++f) {
       const long long q = f * g.fstride + p;
       if (!stage2) out[q] = fma(dt, R[q], Un[q]);
       else out[q] = 0.5 * Un[q] + 0.5 * fma(dt, R[q], U1[q]);
@@ -231,29 +230,32 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
 //      stay in registers; the z stencil is read from a ring of primitive planes in shared memory.
 // Every face flux and every cell reconstruction inside a tile is computed once; 224 of 256 lanes do
 // useful work in every phase.  The ring holds conserved planes loaded by TMA (4-D box: x, y, one z
-// plane, five fields) and converted to primitives in place (a2).
-template <int S>
+// plane, all NF fields) and converted to primitives in place (a2).  NF = 6 adds the radiation energy
+// density (NEXT-1): reconstructed like the other variables, Rusanov flux, untouched by the conversion.
+template <int S, int NF = 5>
 struct StageCfg {
   static constexpr int G = SchemeTraits<S>::G, R = SchemeTraits<S>::R;
   static constexpr int TX = 14, TY = 16, NT = 256;
   static constexpr int BX = TX + 2 * G, BY = TY + 2 * G;      // TMA box
   static constexpr int VS = BX * BY;                          // doubles per field per plane slot
-  static constexpr int SLOT = (5 * VS + 15) / 16 * 16;        // slot stride, multiple of 128 B
+  static constexpr int SLOT = (NF * VS + 15) / 16 * 16;       // slot stride, multiple of 128 B
   // z window of 2R+1 planes.  R >= 2: the oldest plane is not the x/y plane, it is released after the
   // z reconstruction and its slot takes the next plane (no spare slot); otherwise one spare slot.
   static constexpr int NS = (R >= 2) ? 2 * R + 1 : 2 * R + 2;
   static constexpr int NYI = TX * (TY + 2);                   // y reconstruction items
-  static constexpr uint32_t BOX_BYTES = 5u * VS * 8u;
-  static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * 5 * NYI * 8 + NS * 8 + 64 * 8;
+  static constexpr uint32_t BOX_BYTES = (uint32_t)NF * VS * 8u;
+  static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * NF * NYI * 8 + NS * 8 + 64 * 8;
+  // resident CTAs per SM: 2, except WENO with six fields (130 KB of shared memory)
+  static constexpr int CTAS = (SMEM > 113 * 1024) ? 1 : 2;
 };
 
 // Both face values of all five primitives of one cell along one direction; o[s] = ring offset of
 // field 0 at stencil position s - R.  Scheme A applies the positivity fallback (G4).
-template <int S>
-__device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double pl[5], double mi[5]) {
-  constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S>::VS;
+template <int S, int NF>
+__device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double* pl, double* mi) {
+  constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S, NF>::VS;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {
+  for (int v = 0; v < NF; ++v) {
     if (S == SCHEME_A) {
       wenoz_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], ring[o[3] + v * VS],
                  ring[o[4] + v * VS], pl[v], mi[v]);
@@ -264,36 +266,37 @@ __device__ __forceinline__ void recon_item(const double* __restrict__ ring, cons
   if (S == SCHEME_A) {
     if (pl[0] <= 0.0 || pl[4] <= 0.0 || mi[0] <= 0.0 || mi[4] <= 0.0) {
 #pragma unroll
-      for (int v = 0; v < 5; ++v) pl[v] = mi[v] = ring[o[R] + v * VS];
+      for (int v = 0; v < NF; ++v) pl[v] = mi[v] = ring[o[R] + v * VS];     // G19: E_rad follows
     }
   }
 }
 
 // Flux through a face with normal along direction D from (rho,u,v,w,p) face states; result in
 // (rho, mx, my, mz, E) order.
-template <int S, int D>
-__device__ __forceinline__ void face_flux(const double L[5], const double Rr[5], double gamma, double inv_gm1,
-                                          double F[5]) {
+template <int S, int D, int NF>
+__device__ __forceinline__ void face_flux(const double* L, const double* Rr, double gamma, double inv_gm1, double* F) {
   constexpr int n = 1 + D, t1 = 1 + (D + 1) % 3, t2 = 1 + (D + 2) % 3;
   const double WL[5] = { L[0], L[n], L[t1], L[t2], L[4] };
   const double WR[5] = { Rr[0], Rr[n], Rr[t1], Rr[t2], Rr[4] };
-  double f[5];
-  riemann_flux<S>(WL, WR, gamma, inv_gm1, f);
+  double f[5], alpha;
+  riemann_flux<S>(WL, WR, gamma, inv_gm1, f, alpha);
   F[0] = f[0]; F[n] = f[1]; F[t1] = f[2]; F[t2] = f[3]; F[4] = f[4];
+  // NEXT-1 (G19): Rusanov flux of the advected radiation energy density, alpha = max(|u_n| + c_s)
+  if (NF == 6) F[5] = 0.5 * (L[5] * WL[1] + Rr[5] * WR[1]) - 0.5 * alpha * (Rr[5] - L[5]);
 }
 
-template <int S>
-__global__ void __launch_bounds__(256, 2)
+template <int S, int NF>
+__global__ void __launch_bounds__(256, (StageCfg<S, NF>::CTAS))
 stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict__ Usrc, const double* Uaux,
              double* Uout, GridDesc g, DevScalars* sc, StageArgs a) {
-  using C = StageCfg<S>;
+  using C = StageCfg<S, NF>;
   constexpr int G = C::G, R = C::R, TX = C::TX, TY = C::TY, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS,
                 NYI = C::NYI;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);   // dynamic smem base is 1024-B aligned (TMA needs 128)
   double* RMy = ring + NS * SLOT;      // y minus values, item-indexed [v][item]
-  double* Fy = RMy + 5 * NYI;          // y face fluxes: item's upper face
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + 5 * NYI);
+  double* Fy = RMy + NF * NYI;         // y face fluxes: item's upper face
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + NF * NYI);
   double* red = reinterpret_cast<double*>(bars + NS);
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -346,7 +349,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
   for (int z = zb; z <= zb + 2 * rz; ++z) wait_convert(z);
   __syncthreads();
 
-  double zplus[5] = { 0, 0, 0, 0, 0 }, Fzold[5] = { 0, 0, 0, 0, 0 };
+  double zplus[NF] = {}, Fzold[NF] = {};
   double lam_loc = 0.0;
   int bad = 0;
   const bool act3[3] = { g.act[0] != 0, g.act[1] != 0, g.act[2] != 0 };
@@ -360,7 +363,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     const bool late = (znext - NS) >= (kk + ld - rz);
     if (more && !late && tid == 0) { fence_proxy_async(); issue(znext); }
     const int slot_c = ((kk - zb) % NS) * SLOT;        // plane kk (x/y stencils)
-    double Lacc[5] = { 0, 0, 0, 0, 0 };                 // L(U) of the owned cell, accumulated in registers (a5)
+    double Lacc[NF] = {};                             // L(U) of the owned cell, accumulated in registers (a5)
 
     // ---- z: reconstruct plane kk+1 (own column), flux through face kk+1/2 with the carried plus value
     if (az) {
@@ -368,28 +371,28 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
       const int cell = (ty + G) * BX + (tx - 1 + G);
 #pragma unroll
       for (int s = -R; s <= R; ++s) o[s + R] = ((kk + 1 + s - zb) % NS) * SLOT + cell;
-      double pl[5], mi[5];
-      recon_item<S>(ring, o, pl, mi);
+      double pl[NF], mi[NF];
+      recon_item<S, NF>(ring, o, pl, mi);
       if (kk >= k0 - 1) {
-        double F[5];
-        face_flux<S, 2>(zplus, mi, gamma, inv_gm1, F);
+        double F[NF];
+        face_flux<S, 2, NF>(zplus, mi, gamma, inv_gm1, F);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) { Lacc[v] = (Fzold[v] - F[v]) * idz; Fzold[v] = F[v]; }
+        for (int v = 0; v < NF; ++v) { Lacc[v] = (Fzold[v] - F[v]) * idz; Fzold[v] = F[v]; }
       }
 #pragma unroll
-      for (int v = 0; v < 5; ++v) zplus[v] = pl[v];
+      for (int v = 0; v < NF; ++v) zplus[v] = pl[v];
     }
     // ---- y: reconstruct the 14 x (rows+2) items of plane kk; minus values to shared memory
-    double plY[5] = { 0, 0, 0, 0, 0 };
+    double plY[NF] = {};
     if (doxy && yitem) {
       int o[2 * R + 1];
       const int cell = slot_c + (y_c - 1 + G) * BX + (y_ix + G);
 #pragma unroll
       for (int s = -R; s <= R; ++s) o[s + R] = cell + s * BX;
-      double mi[5];
-      recon_item<S>(ring, o, plY, mi);
+      double mi[NF];
+      recon_item<S, NF>(ring, o, plY, mi);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) RMy[v * NYI + tid] = mi[v];
+      for (int v = 0; v < NF; ++v) RMy[v * NYI + tid] = mi[v];
     }
     __syncthreads();                                                             // barrier 1
     if (more && late && tid == 0) { fence_proxy_async(); issue(znext); }
@@ -397,37 +400,39 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     // own-cell conserved values for the RK combination, consumed after barrier 2.  Scheme A issues the
     // loads here; scheme B after the x phase (measured: holding 10-20 registers through the x phase
     // costs B 4 %, while the later issue costs A 2 %).
-    double uc[5] = { 0, 0, 0, 0, 0 }, ua[5] = { 0, 0, 0, 0, 0 };
+    double uc[NF] = {}, ua[NF] = {};
     long long pc = 0;
     auto load_own = [&]() {
       if (doxy && mine) {
         pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
         if (a.mode != MODE_RESID) {
 #pragma unroll
-          for (int v = 0; v < 5; ++v) uc[v] = Usrc[v * g.fstride + pc];
+          for (int v = 0; v < NF; ++v) uc[v] = Usrc[v * g.fstride + pc];
         }
         if (a.mode == MODE_STAGE2 || (a.mode == MODE_RESID && !a.first)) {
 #pragma unroll
-          for (int v = 0; v < 5; ++v) ua[v] = Uaux[v * g.fstride + pc];
+          for (int v = 0; v < NF; ++v) ua[v] = Uaux[v * g.fstride + pc];
         }
       }
     };
     if (S == SCHEME_A) load_own();
     // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
     if (doxy && ax) {
-      double pl[5] = { 1, 0, 0, 0, 1 }, mi[5] = { 1, 0, 0, 0, 1 }, mr[5], F[5];
+      double pl[NF], mi[NF], mr[NF], F[NF];
+#pragma unroll
+      for (int v = 0; v < NF; ++v) pl[v] = mi[v] = (v == 0 || v == 4) ? 1.0 : 0.0;
       if (ty < rows) {
         int o[2 * R + 1];
         const int cell = slot_c + (ty + G) * BX + (tx - 1 + G);
 #pragma unroll
         for (int s = -R; s <= R; ++s) o[s + R] = cell + s;
-        recon_item<S>(ring, o, pl, mi);
+        recon_item<S, NF>(ring, o, pl, mi);
       }
 #pragma unroll
-      for (int v = 0; v < 5; ++v) mr[v] = __shfl_down_sync(0xffffffffu, mi[v], 1, 16);   // minus of cell tx
-      face_flux<S, 0>(pl, mr, gamma, inv_gm1, F);                                        // face right of cell tx-1
+      for (int v = 0; v < NF; ++v) mr[v] = __shfl_down_sync(0xffffffffu, mi[v], 1, 16);   // minus of cell tx
+      face_flux<S, 0, NF>(pl, mr, gamma, inv_gm1, F);                                        // face right of cell tx-1
 #pragma unroll
-      for (int v = 0; v < 5; ++v) {
+      for (int v = 0; v < NF; ++v) {
         const double Fl = __shfl_up_sync(0xffffffffu, F[v], 1, 16);                      // face left of cell tx-1
         Lacc[v] -= (F[v] - Fl) * idx;
       }
@@ -435,21 +440,21 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     if (S != SCHEME_A) load_own();
     // ---- y fluxes: face above item (between item and item + TX)
     if (doxy && yface) {
-      double mr[5], F[5];
+      double mr[NF], F[NF];
 #pragma unroll
-      for (int v = 0; v < 5; ++v) mr[v] = RMy[v * NYI + tid + TX];
-      face_flux<S, 1>(plY, mr, gamma, inv_gm1, F);
+      for (int v = 0; v < NF; ++v) mr[v] = RMy[v * NYI + tid + TX];
+      face_flux<S, 1, NF>(plY, mr, gamma, inv_gm1, F);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) Fy[v * NYI + tid] = F[v];
+      for (int v = 0; v < NF; ++v) Fy[v * NYI + tid] = F[v];
     }
     __syncthreads();                                                             // barrier 2
 
     // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
     if (doxy && mine) {
-      double out[5];
+      double out[NF];
       const int yi = ty * TX + (tx - 1);               // item of cell (tx-1, ty-1): its upper face is our lower face
 #pragma unroll
-      for (int v = 0; v < 5; ++v) {
+      for (int v = 0; v < NF; ++v) {
         double L = Lacc[v];
         if (ay) L -= (Fy[v * NYI + yi + TX] - Fy[v * NYI + yi]) * idy;
         if (a.mode == MODE_STAGE1) out[v] = fma(dt, L, uc[v]);

@@ -22,7 +22,8 @@ VARIANT_FUSED, VARIANT_PERDIR = 0, 1
 EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard_max_dt", "hard_destroy",
            "hard_set_spacing", "hard_set_scheme", "hard_set_variant", "hard_set_stream", "hard_workspace_bytes",
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
-           "hard_stage_time", "hard_probe_fp64_peak"]
+           "hard_stage_time", "hard_probe_fp64_peak", "hard_enable_radiation", "hard_set_rad_energy",
+           "hard_get_rad_energy"]
 
 _lib = None
 
@@ -58,6 +59,9 @@ def lib():
     L.hard_launch_count.restype = ctypes.c_longlong
     L.hard_launch_count.argtypes = [vp]
     L.hard_stage_time.argtypes = [vp, c_int, ctypes.POINTER(c_dbl), ctypes.POINTER(ctypes.c_longlong)]
+    L.hard_enable_radiation.argtypes = [vp]
+    L.hard_set_rad_energy.argtypes = [vp, dp]
+    L.hard_get_rad_energy.argtypes = [vp, dp]
     L.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(c_dbl), ctypes.POINTER(c_dbl)]
     _lib = L
     return L
@@ -91,7 +95,7 @@ class Hard:
     """One simulation (hard_ctx).  Fields are (nz, ny, nx) float64, conserved (rho, mx, my, mz, E)."""
 
     def __init__(self, nx, ny, nz, gamma, bc, scheme=SCHEME_WENO5Z_HLL, variant=VARIANT_FUSED, spacing=None,
-                 torch_workspace=True, stream=None):
+                 torch_workspace=True, stream=None, radiation=False):
         self.L = lib()
         self.n = (nx, ny, nz)
         self.shape = (nz, ny, nx)
@@ -100,6 +104,8 @@ class Hard:
             raise HardError(ERR_CUDA, self.L.hard_last_error(None).decode())
         self._chk(self.L.hard_set_scheme(self.h, scheme))
         self._chk(self.L.hard_set_variant(self.h, variant))
+        if radiation:
+            self._chk(self.L.hard_enable_radiation(self.h))
         if spacing is not None:
             self._chk(self.L.hard_set_spacing(self.h, *map(float, spacing)))
         self.ws = None
@@ -149,6 +155,15 @@ class Hard:
         return v.value
 
     # ---- extensions
+    def set_rad_energy(self, er):
+        self._chk(self.L.hard_set_rad_energy(self.h, _ptr(er)))
+
+    def get_rad_energy(self, out=None):
+        if out is None:
+            out = np.empty(self.shape, dtype=np.float64)
+        self._chk(self.L.hard_get_rad_energy(self.h, _ptr(out)))
+        return out
+
     def set_variant(self, variant):
         self._chk(self.L.hard_set_variant(self.h, variant))
 

@@ -135,3 +135,40 @@ def test_kelvin_helmholtz_2d(scheme):
     w = wl.kelvin_helmholtz(256, nsteps=100)
     _check(w, scheme, hard.VARIANT_FUSED, 1, TOL_1)
     _check(w, scheme, hard.VARIANT_FUSED, 100, TOL_100)
+
+
+# ---------------------------------------------------------------- NEXT-1: advected radiation energy density
+def _check_rad(w, er, scheme, variant, nsteps, tol):
+    import oracle
+    st = [np.ascontiguousarray(a, dtype=np.float64) for a in w.state]
+    o = oracle.Oracle(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing, radiation=True)
+    o.set_state(*st)
+    o.set_rad_energy(er)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing, radiation=True)
+    h.set_state(*st)
+    h.set_rad_energy(np.ascontiguousarray(er))
+    assert abs(h.max_dt() - o.max_dt()) <= TOL_DT * o.max_dt()
+    o.step(w.cfl, nsteps)
+    h.step(w.cfl, nsteps)
+    errs = field_errors(h.get_state() + [h.get_rad_energy()], o.get_state() + [o.get_rad_energy()])
+    assert max(errs) <= tol, errs
+    assert np.abs(o.get_rad_energy() - er).max() > 0
+    h.close()
+    o.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("n,bc", [((37, 21, 19), wl.BC_PERIODIC), ((45, 30, 1), wl.BC_REFLECT), ((131, 1, 1), wl.BC_OUTFLOW)])
+def test_radiation_energy_advection(scheme, variant, n, bc):
+    w = _random_workload(n, bc, seed=11 + sum(n), spacing=(0.1, 0.07, 0.13))
+    er = 1.0 + 0.5 * np.random.default_rng(5).random(n[::-1])
+    _check_rad(w, er, scheme, variant, 1, TOL_1)
+    _check_rad(w, er, scheme, variant, 25, TOL_100)
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_radiation_energy_turbulence_100_steps(scheme):
+    w = wl.turbulence(40, nsteps=100)
+    er = 1.0 + 0.3 * np.sin(2 * np.pi * np.arange(40) / 40.0)[None, None, :] * np.ones((40, 40, 40))
+    _check_rad(w, er, scheme, hard.VARIANT_FUSED, 100, TOL_100)
