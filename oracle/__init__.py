@@ -74,6 +74,7 @@ def lib():
         L.oracle_enable_radiation.argtypes = [vp]
         L.oracle_set_rad_energy.argtypes = [vp, dp]
         L.oracle_get_rad_energy.argtypes = [vp, dp]
+        L.oracle_set_source.argtypes = [vp] + [ctypes.c_double] * 4
         L.oracle_rusanov.restype = ctypes.c_double
         L.oracle_rusanov.argtypes = [ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_double]
         _lib = L
@@ -138,6 +139,9 @@ class Oracle:
     def set_rad_energy(self, er):
         a = np.ascontiguousarray(er, dtype=np.float64).reshape(self.shape)
         self._chk(self.L.oracle_set_rad_energy(self.h, _dp(a)), "set_rad_energy")
+
+    def set_source(self, kappa, c_light, a_rad, cv):
+        self._chk(self.L.oracle_set_source(self.h, float(kappa), float(c_light), float(a_rad), float(cv)), "set_source")
 
     def get_rad_energy(self):
         out = np.empty(self.shape, dtype=np.float64)

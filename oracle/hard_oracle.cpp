@@ -22,6 +22,8 @@
 //   ghost entities of the N-array topology                        P:64             (BCs: G10, G17)
 //   radiation energy density advected with the fluid, Rusanov    P:93 eq.2 (4th row), eq.14 LHS,
 //   (local Lax-Friedrichs) flux                                   P:151            (NEXT-1; G19)
+//   radiative heating q = c kappa rho (E_rad - a T^4), operator   P:66, eq.4,6
+//   split after the advection step, backward Euler                                 (NEXT-3; G20)
 // Every place where the paper is silent is a DESIGN.md reading (G1..G13) and is marked below.
 //
 // Pins (tests/test_oracle_*.py, all -m "not gpu"): exact Sod / LeBlanc Riemann solutions and L1
@@ -185,6 +187,8 @@ struct Ctx {
   double gamma, d[3];
   int nf;                   // 5, or 6 with the advected radiation energy density (NEXT-1)
   std::vector<double> U[6], U1[6];
+  int src_on;               // NEXT-3: radiative heating/cooling source after each advection step
+  double src_kappa, src_c, src_a, src_cv;
   double lambda, t;
   long long steps;
   long long fallbacks;      // G4 positivity fallbacks taken so far
@@ -326,6 +330,40 @@ void rhs(Ctx* c, const std::vector<double> V[6], std::vector<double> Lout[6]) {
   }
 }
 
+// NEXT-3 (G20): the pointwise source update of the paper's operator split ("advection, diffusion, source
+// updates") restricted to the heating rate q = c kappa rho (E_rad - a T^4) (eq.6; force and
+// diffusion out of scope): d_t e = q, d_t E_rad = -q (eq.4), T = e / (rho c_v) (ideal gas).  Backward
+// Euler over dt conserves e + E_rad exactly: solve g(x) = x - e - dt c kappa rho (E_tot - x - a (x/(rho c_v))^4) = 0
+// for the new internal energy density x by Newton's method, safeguarded by the bracket [0, E_tot] on which
+// g is increasing and changes sign.
+void apply_source(Ctx* c, double dt) {
+  for (int k = 0; k < c->n[2]; ++k)
+    for (int j = 0; j < c->n[1]; ++j)
+      for (int i = 0; i < c->n[0]; ++i) {
+        long p = c->idx(i, j, k);
+        double rho = c->U[0][p];
+        double ke = 0.5 * sum3sym(c->U[1][p] * c->U[1][p], c->U[2][p] * c->U[2][p], c->U[3][p] * c->U[3][p]) / rho;
+        double e = c->U[4][p] - ke, Er = c->U[5][p];
+        double Etot = e + Er;
+        double beta = dt * c->src_c * c->src_kappa * rho;
+        double rcv = rho * c->src_cv;
+        double lo = 0.0, hi = Etot, x = e < 0.0 ? 0.0 : (e > Etot ? Etot : e);
+        for (int it = 0; it < 200; ++it) {
+          double T = x / rcv, T2 = T * T, T4 = T2 * T2;
+          double gx = (x - e) - beta * ((Etot - x) - c->src_a * T4);
+          if (gx > 0.0) hi = x; else lo = x;
+          double dg = 1.0 + beta * (1.0 + 4.0 * c->src_a * T2 * T / rcv);
+          double xn = x - gx / dg;
+          if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);            // Newton left the bracket: bisect
+          double dx = std::fabs(xn - x);
+          x = xn;
+          if (dx <= 1e-15 * std::fabs(x)) break;
+        }
+        c->U[4][p] = x + ke;
+        c->U[5][p] = Etot - x;
+      }
+}
+
 // One Heun / SSP-RK2 step with a given dt (Table 2; Shu-Osher form, G7).
 void step_dt(Ctx* c, double dt) {
   std::vector<double> L[6];
@@ -346,6 +384,7 @@ void step_dt(Ctx* c, double dt) {
         for (int f = 0; f < c->nf; ++f)
           c->U[f][p] = 0.5 * c->U[f][p] + 0.5 * (c->U1[f][p] + dt * L[f][q]);
       }
+  if (c->src_on) apply_source(c, dt);
   if (c->check) c->lambda = maxwavespeed(c, c->U);
   c->t += dt;
   c->steps += 1;
@@ -359,7 +398,7 @@ void* oracle_create(int nx, int ny, int nz, double gamma, int bc) {
   if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || (bc != BC_PERIODIC && bc != BC_OUTFLOW && bc != BC_REFLECT)) return nullptr;
   Ctx* c = new Ctx();
   c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
-  c->gamma = gamma; c->bc = bc; c->scheme = SCHEME_A; c->nf = 5;
+  c->gamma = gamma; c->bc = bc; c->scheme = SCHEME_A; c->nf = 5; c->src_on = 0;
   c->d[0] = 1.0 / nx; c->d[1] = 1.0 / ny; c->d[2] = 1.0 / nz;
   c->lambda = 0.0; c->t = 0.0; c->steps = 0; c->fallbacks = 0;
   c->status = ORC_OK; c->check = 1;
@@ -408,6 +447,14 @@ int oracle_get_rad_energy(void* h, double* er) {
       for (int i = 0; i < c->n[0]; ++i)
         er[(long)i + (long)c->n[0] * ((long)j + (long)c->n[1] * k)] = c->U[5][c->idx(i, j, k)];
   return c->status;
+}
+
+// NEXT-3: heating/cooling source after every step; needs oracle_enable_radiation.  cv: T = e / (rho cv).
+int oracle_set_source(void* h, double kappa, double c_light, double a_rad, double cv) {
+  Ctx* c = (Ctx*)h;
+  if (!c || c->nf != 6 || !(kappa >= 0.0 && c_light > 0.0 && a_rad > 0.0 && cv > 0.0)) return ORC_ERR_ARG;
+  c->src_on = 1; c->src_kappa = kappa; c->src_c = c_light; c->src_a = a_rad; c->src_cv = cv;
+  return ORC_OK;
 }
 
 int oracle_set_scheme(void* h, int scheme) {
