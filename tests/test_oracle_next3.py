@@ -77,7 +77,7 @@ def test_one_backward_euler_step_is_the_root_of_its_equation():
     o.step_dt(dt, 1)
     beta = dt * C_LIGHT * KAPPA * RHO
     g = lambda x: (x - e0) - beta * ((e0 + er0 - x) - A_RAD * (x / (RHO * CV)) ** 4)
-    root = brentq(g, 0.0, e0 + er0, xtol=0.0, rtol=4e-16)
+    root = brentq(g, 0.0, e0 + er0, xtol=1e-300, rtol=1e-15)
     assert abs(_e_of(o, vel) - root) <= 1e-13 * root
     s = o.get_state()
     for f, v in zip((0, 1, 2, 3), (RHO, RHO * vel[0], RHO * vel[1], RHO * vel[2])):
