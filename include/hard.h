@@ -90,6 +90,12 @@ int hard_enable_radiation(hard_ctx*);
 int hard_set_rad_energy(hard_ctx*, const double* e_rad);
 int hard_get_rad_energy(hard_ctx*, double* e_rad);
 
+/* NEXT-3: after every Heun step apply the pointwise radiative heating / cooling source of the
+ * paper's operator split: q = c kappa rho (E_rad - a T^4) (eq.6), d_t e = q, d_t E_rad = -q
+ * (eq.4), T = e / (rho cv) for the ideal gas, backward Euler over the step's dt (G20); e + E_rad is
+ * conserved exactly.  Needs hard_enable_radiation.  kappa >= 0, the other parameters > 0 (any unit system). */
+int hard_set_source(hard_ctx*, double kappa, double c_light, double a_rad, double cv);
+
 /* HARD_VARIANT_*; may be switched at any time between steps (same state buffers). */
 int hard_set_variant(hard_ctx*, int variant);
 

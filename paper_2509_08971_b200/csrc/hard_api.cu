@@ -31,6 +31,8 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct hard_ctx {
   GridDesc g;
   int scheme = HARD_SCHEME_WENO5Z_HLL, variant = HARD_VARIANT_FUSED;
+  bool src_on = false;              // NEXT-3: heating/cooling source after every step (hard_set_source)
+  SourceParams src{};
   int nf = 5;                       // 6 with the advected radiation energy density (hard_enable_radiation)
   cudaStream_t stream = 0;
   void* ws = nullptr;
@@ -235,6 +237,7 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
   StageArgs a;
   a.mode = mode; a.dirmask = dirmask; a.first = first; a.cur = (int)(c->steps_enq & 1);
   a.cfl = cfl; a.dt_fixed = dt_fixed;
+  a.skip_cfl = c->src_on ? 1 : 0;
   const bool zact = g.act[2] && (dirmask & 4);
   a.Lz = zact ? c->Lz : (g.n[2] + ((g.n[2] + 63) / 64) - 1) / ((g.n[2] + 63) / 64);   // z inactive: chunks of <= 64 planes
   dim3 grid((g.n[0] + 13) / 14, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
@@ -247,6 +250,12 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
 #undef HARD_LAUNCH
   if ((rc = after_launch(c, "stage_kernel"))) return rc;
   return prof_end(c);
+}
+
+int launch_source(hard_ctx* c, double cfl, double dt_fixed) {
+  const long long N = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2];
+  source_kernel<<<small_grid(c, N), 256, 0, c->stream>>>(c->U, c->g, c->sc, c->src, (int)(c->steps_enq & 1), cfl, dt_fixed);
+  return after_launch(c, "source_kernel");
 }
 
 int launch_axpy(hard_ctx* c, int stage2, double cfl, double dt_fixed) {
@@ -281,13 +290,15 @@ int do_steps(hard_ctx* c, double cfl, double dt_fixed, int nsteps) {
       if ((rc = launch_stage(c, c->tmU, c->U, nullptr, c->U1, MODE_STAGE1, 7, 0, cfl, dt_fixed))) return rc;
       if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
       if ((rc = launch_stage(c, c->tmU1, c->U1, c->U, c->U, MODE_STAGE2, 7, 0, cfl, dt_fixed))) return rc;
+      if (c->src_on && (rc = launch_source(c, cfl, dt_fixed))) return rc;
     } else {
       if ((rc = perdir_residual(c, c->tmU, c->U, cfl, dt_fixed))) return rc;
       if ((rc = launch_axpy(c, 0, cfl, dt_fixed))) return rc;
       if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
       if ((rc = perdir_residual(c, c->tmU1, c->U1, cfl, dt_fixed))) return rc;
       if ((rc = launch_axpy(c, 1, cfl, dt_fixed))) return rc;
-      if ((rc = launch_cfl(c, c->U, (int)((c->steps_enq & 1) ^ 1)))) return rc;
+      if (c->src_on) { if ((rc = launch_source(c, cfl, dt_fixed))) return rc; }
+      else if ((rc = launch_cfl(c, c->U, (int)((c->steps_enq & 1) ^ 1)))) return rc;
     }
     c->steps_enq++;
   }
@@ -413,6 +424,15 @@ int hard_get_rad_energy(hard_ctx* c, double* er) {
   if (rc) return rc;
   DevScalars h;
   return sync_status(c, &h);
+}
+
+int hard_set_source(hard_ctx* c, double kappa, double c_light, double a_rad, double cv) {
+  if (!c) return HARD_ERR_ARG;
+  if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_set_source: call hard_enable_radiation first");
+  if (!(kappa >= 0.0 && c_light > 0.0 && a_rad > 0.0 && cv > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_source: bad parameter");
+  c->src_on = true;
+  c->src.kappa = kappa; c->src.c_light = c_light; c->src.a_rad = a_rad; c->src.cv = cv;
+  return HARD_OK;
 }
 
 int hard_set_variant(hard_ctx* c, int variant) {

@@ -45,6 +45,7 @@ struct StageArgs {
   int Lz;           // planes per z-chunk
   int cur;          // lam_bits[cur] is lambda(U^n); stage 2 accumulates into lam_bits[cur^1]
   double cfl, dt_fixed;   // dt = dt_fixed > 0 ? dt_fixed : cfl / lambda
+  int skip_cfl;           // stage 2: leave the max-wavespeed reduction to the source kernel (NEXT-3)
 };
 
 __device__ __forceinline__ double step_dt(const DevScalars* sc, int cur, double cfl, double dt_fixed) {
@@ -187,6 +188,59 @@ __global__ void axpy_kernel(const double* __restrict__ Un, const double* __restr
       else out[q] = 0.5 * Un[q] + 0.5 * fma(dt, R[q], U1[q]);
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------- NEXT-3: source update
+// Pointwise radiative heating / cooling (eq.6; d_t e = q, d_t E_rad = -q, eq.4), operator-split
+// after the advection step, backward Euler over dt (G20): the new internal energy density x solves
+// g(x) = x - e - dt c kappa rho (E_tot - x - a (x/(rho c_v))^4) = 0 on [0, E_tot] (g increasing): Newton,
+// bisecting when an iterate leaves the bracket.  e + E_rad is conserved exactly.  HBM-bound (6 fields read,
+// 2 written: 64 B per cell).  It also carries the step's max-wavespeed reduction (a7), since the source
+// changes the pressure.
+struct SourceParams { double kappa, c_light, a_rad, cv; };
+
+__global__ void source_kernel(double* __restrict__ U, GridDesc g, DevScalars* sc, SourceParams sp, int cur, double cfl,
+                              double dt_fixed) {
+  __shared__ double red[64];
+  const double dt = step_dt(sc, cur, cfl, dt_fixed);
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  const double gm1 = g.gamma - 1.0;
+  const bool act3[3] = { g.act[0] != 0, g.act[1] != 0, g.act[2] != 0 };
+  double lam = 0.0;
+  int bad = 0;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < N;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % g.n[0]);
+    const long long r = idx / g.n[0];
+    const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+    const long long p = cell_addr(g, i, j, k);
+    double Uc[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) Uc[f] = U[f * g.fstride + p];
+    const double Er = U[5 * g.fstride + p];
+    const double rho = Uc[0];
+    const double ke = 0.5 * (Uc[1] * Uc[1] + Uc[2] * Uc[2] + Uc[3] * Uc[3]) / rho;
+    const double e = Uc[4] - ke, Etot = e + Er;
+    const double beta = dt * sp.c_light * sp.kappa * rho, rcv = rho * sp.cv, inv_rcv = 1.0 / rcv;
+    double lo = 0.0, hi = Etot, x = e < 0.0 ? 0.0 : (e > Etot ? Etot : e);
+    for (int it = 0; it < 200; ++it) {
+      const double T = x * inv_rcv, T2 = T * T, T4 = T2 * T2;
+      const double gx = (x - e) - beta * ((Etot - x) - sp.a_rad * T4);
+      if (gx > 0.0) hi = x; else lo = x;
+      const double dg = 1.0 + beta * (1.0 + 4.0 * sp.a_rad * T2 * T * inv_rcv);
+      double xn = x - gx / dg;
+      if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);
+      const double dx = fabs(xn - x);
+      x = xn;
+      if (dx <= 1e-15 * fabs(x)) break;
+    }
+    Uc[4] = x + ke;
+    U[4 * g.fstride + p] = Uc[4];
+    U[5 * g.fstride + p] = Etot - x;
+    const double l = cell_lambda(Uc, g.gamma, gm1, g.inv_d, act3);
+    if (l < 0.0 || !(Etot - x >= 0.0)) bad = 1; else lam = fmax(lam, l);
+  }
+  block_max_to_slot(lam, bad, sc, cur ^ 1, red);
 }
 
 // ------------------------------------------------------------------------------------------- TMA / mbarrier PTX
@@ -462,7 +516,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
         else out[v] = a.first ? L : ua[v] + L;
         Uout[v * g.fstride + pc] = out[v];
       }
-      if (a.mode == MODE_STAGE2) {
+      if (a.mode == MODE_STAGE2 && !a.skip_cfl) {
         const double l = cell_lambda(out, gamma, gm1, g.inv_d, act3);
         if (l < 0.0) bad = 1; else lam_loc = fmax(lam_loc, l);
       }
@@ -470,7 +524,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     if (more) wait_convert(znext);
     __syncthreads();                                                             // barrier 3
   }
-  if (a.mode == MODE_STAGE2) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
+  if (a.mode == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
 }
 
 }  // namespace hard

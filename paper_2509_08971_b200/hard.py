@@ -23,7 +23,7 @@ EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard
            "hard_set_spacing", "hard_set_scheme", "hard_set_variant", "hard_set_stream", "hard_workspace_bytes",
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
            "hard_stage_time", "hard_probe_fp64_peak", "hard_enable_radiation", "hard_set_rad_energy",
-           "hard_get_rad_energy"]
+           "hard_get_rad_energy", "hard_set_source"]
 
 _lib = None
 
@@ -62,6 +62,7 @@ def lib():
     L.hard_enable_radiation.argtypes = [vp]
     L.hard_set_rad_energy.argtypes = [vp, dp]
     L.hard_get_rad_energy.argtypes = [vp, dp]
+    L.hard_set_source.argtypes = [vp, c_dbl, c_dbl, c_dbl, c_dbl]
     L.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(c_dbl), ctypes.POINTER(c_dbl)]
     _lib = L
     return L
@@ -155,6 +156,9 @@ class Hard:
         return v.value
 
     # ---- extensions
+    def set_source(self, kappa, c_light, a_rad, cv):
+        self._chk(self.L.hard_set_source(self.h, float(kappa), float(c_light), float(a_rad), float(cv)))
+
     def set_rad_energy(self, er):
         self._chk(self.L.hard_set_rad_energy(self.h, _ptr(er)))
 

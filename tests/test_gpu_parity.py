@@ -172,3 +172,56 @@ def test_radiation_energy_turbulence_100_steps(scheme):
     w = wl.turbulence(40, nsteps=100)
     er = 1.0 + 0.3 * np.sin(2 * np.pi * np.arange(40) / 40.0)[None, None, :] * np.ones((40, 40, 40))
     _check_rad(w, er, scheme, hard.VARIANT_FUSED, 100, TOL_100)
+
+
+# ---------------------------------------------------------------- NEXT-3: radiative heating / cooling source
+def _check_source(w, er, params, scheme, variant, nsteps, tol, dt=None):
+    import oracle
+    st = [np.ascontiguousarray(a, dtype=np.float64) for a in w.state]
+    o = oracle.Oracle(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing, radiation=True)
+    o.set_source(*params)
+    o.set_state(*st)
+    o.set_rad_energy(er)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing, radiation=True)
+    h.set_source(*params)
+    h.set_state(*st)
+    h.set_rad_energy(np.ascontiguousarray(er))
+    if dt is None:
+        o.step(w.cfl, nsteps)
+        h.step(w.cfl, nsteps)
+    else:
+        o.step_dt(dt, nsteps)
+        h.step_dt(dt, nsteps)
+    errs = field_errors(h.get_state() + [h.get_rad_energy()], o.get_state() + [o.get_rad_energy()])
+    assert max(errs) <= tol, errs
+    assert abs(h.max_dt() - o.max_dt()) <= max(10 * tol, 1e-12) * o.max_dt()
+    assert abs(h.time()[0] - o.time()[0]) <= 1e-12 * o.time()[0]
+    assert np.abs(o.get_rad_energy() - er).max() > 0
+    h.close()
+    o.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_source_on_random_state(scheme, variant):
+    n = (37, 21, 19)
+    w = _random_workload(n, wl.BC_PERIODIC, seed=77, spacing=(0.1, 0.07, 0.13))
+    er = 1.0 + 0.5 * np.random.default_rng(6).random(n[::-1])
+    params = (0.7, 3.0, 0.5, 1.2)                  # kappa, c, a, cv in code units
+    _check_source(w, er, params, scheme, variant, 1, TOL_1)
+    _check_source(w, er, params, scheme, variant, 25, TOL_100)
+
+
+@pytest.mark.parametrize("T0", [11.0, 1.1e9])
+def test_paper_heating_cooling_cases(T0):
+    """P:209-211 in cgs units: rho = 1e-7, mu = 0.6, kappa = 0.4, T_rad = 3.4e6 K, gas at 11 K / 1.1e9 K."""
+    c_light, a_rad, k_b, m_p = 2.99792458e10, 7.5657e-15, 1.380649e-16, 1.67262192e-24
+    gamma, rho, cv = 5.0 / 3.0, 1e-7, 1.380649e-16 / ((5.0 / 3.0 - 1.0) * 0.6 * 1.67262192e-24)
+    n = (20, 18, 1)
+    e0 = rho * cv * T0
+    z = np.zeros(n[::-1])
+    w = wl.Workload("heat", n, gamma, wl.BC_PERIODIC, (1.0, 1.0, 1.0), 0.4, nsteps=20,
+                    state=[z + rho, z.copy(), z.copy(), z.copy(), z + e0])
+    er = z + a_rad * 3.4e6 ** 4
+    t_end = 2e-7 if T0 < 1e6 else 2e-10
+    _check_source(w, er, (0.4, c_light, a_rad, cv), hard.SCHEME_WENO5Z_HLL, hard.VARIANT_FUSED, 20, TOL_100, dt=t_end / 20)

@@ -100,4 +100,4 @@ def test_zero_opacity_is_a_no_op():
         outs.append(o.get_state() + [o.get_rad_energy()])
         o.close()
     for a, b in zip(*outs):
-        assert np.abs(a - b).max() <= 1e-15 * np.abs(a).max()
+        assert np.abs(a - b).max() <= 1e-13 * np.abs(a).max()      # (E - ke) + ke rounds once per step
