@@ -1,0 +1,131 @@
+"""GPU tests of the C-ABI semantics beyond plain stepping (-m gpu): variant switching, re-setting the state,
+spacing changes, device-resident latching of a non-physical state, non-default streams, library-owned workspace,
+stage timing and launch counting."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2509_08971_b200 import hard
+from paper_2509_08971_b200 import workloads as wl
+
+from _parity import field_errors
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_run(w, scheme, nsteps, spacing=None):
+    o = oracle.Oracle(*w.n, w.gamma, w.bc, scheme=scheme, spacing=spacing or w.spacing)
+    o.set_state(*w.state)
+    o.step(w.cfl, nsteps)
+    out = o.get_state()
+    dt = o.max_dt()
+    o.close()
+    return out, dt
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_variant_switch_mid_run_and_state_reset(scheme):
+    w = wl.turbulence(24, nsteps=6)
+    ref, dt_ref = _oracle_run(w, scheme, 6)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+    h.set_state(*w.state)
+    h.step(w.cfl, 2)
+    h.set_variant(hard.VARIANT_PERDIR)
+    h.step(w.cfl, 2)
+    h.set_variant(hard.VARIANT_FUSED)
+    h.step(w.cfl, 2)
+    assert max(field_errors(h.get_state(), ref)) <= 1e-11
+    assert abs(h.max_dt() - dt_ref) <= 1e-11 * dt_ref
+    assert h.time()[1] == 6
+    # a second hard_set_state restarts the clock and reproduces the run
+    h.set_state(*w.state)
+    assert h.time() == (0.0, 0)
+    h.step(w.cfl, 6)
+    assert max(field_errors(h.get_state(), ref)) <= 1e-11
+    h.close()
+
+
+def test_set_spacing_after_state_reevaluates_lambda():
+    w = wl.turbulence(16, nsteps=1)
+    sp2 = (0.5, 0.25, 0.125)
+    h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)
+    h.set_state(*w.state)
+    h._chk(h.L.hard_set_spacing(h.h, *sp2))
+    o = oracle.Oracle(*w.n, w.gamma, w.bc, spacing=sp2)
+    o.set_state(*w.state)
+    assert abs(h.max_dt() - o.max_dt()) <= 1e-14 * o.max_dt()
+    h.step(w.cfl, 2)
+    o.step(w.cfl, 2)
+    assert max(field_errors(h.get_state(), o.get_state())) <= 1e-12
+    h.close()
+    o.close()
+
+
+def test_nonphysical_state_is_latched_on_the_device_and_surfaced():
+    # a huge fixed dt drives the density negative inside hard_step; nothing returns to the host until a sync
+    w = wl.sod(64)
+    h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)
+    h.set_state(*w.state)
+    h.step_dt(1.0, 2)                       # enqueue only: no error yet
+    with pytest.raises(hard.HardError) as e:
+        h.get_state()
+    assert e.value.code == hard.ERR_NONPHYSICAL
+    with pytest.raises(hard.HardError):
+        h.max_dt()
+    h.set_state(*w.state)                   # a fresh state clears the latch
+    h.step(w.cfl, 1)
+    h.get_state()
+    h.close()
+
+
+def test_non_default_stream_and_library_owned_workspace():
+    import torch
+    w = wl.turbulence(20, nsteps=3)
+    ref, _ = _oracle_run(w, 0, 3)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)          # binds torch's current stream = s
+        h.set_state(*w.state)
+        h.step(w.cfl, 3)
+        out = h.get_state()
+    assert max(field_errors(out, ref)) <= 1e-11
+    h.close()
+    h2 = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing, torch_workspace=False)   # cudaMalloc'ed by the library
+    assert h2.workspace_bytes() > 3 * 5 * 20 ** 3 * 8
+    h2.set_state(*w.state)
+    h2.step(w.cfl, 3)
+    assert max(field_errors(h2.get_state(), ref)) <= 1e-11
+    h2.close()
+
+
+def test_launch_count_and_stage_time():
+    w = wl.turbulence(32, nsteps=4)
+    h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)
+    h.set_state(*w.state)
+    n0 = h.launch_count()
+    h.stage_time(reset=True)
+    h.step(w.cfl, 4)
+    ms, n = h.stage_time(reset=False)
+    assert h.launch_count() - n0 == 4 * 4          # per step: ghost, stage 1, ghost, stage 2
+    assert n == 8 and ms > 0.0
+    h.set_variant(hard.VARIANT_PERDIR)
+    n1 = h.launch_count()
+    h.step(w.cfl, 1)
+    assert h.launch_count() - n1 == 2 + 6 + 2 + 1   # 2 ghost fills, 6 direction passes, 2 axpy, 1 CFL
+    h.close()
+
+
+def test_argument_errors():
+    h = hard.Hard(8, 8, 8, 1.4, 0)
+    assert h.L.hard_step(h.h, -1.0, 1) == hard.ERR_ARG
+    assert h.L.hard_step_dt(h.h, 0.0, 1) == hard.ERR_ARG
+    assert h.L.hard_set_spacing(h.h, 0.0, 1.0, 1.0) == hard.ERR_ARG
+    assert h.L.hard_set_variant(h.h, 7) == hard.ERR_ARG
+    assert h.L.hard_set_rad_energy(h.h, 0) == hard.ERR_ARG
+    assert h.L.hard_set_source(h.h, 1.0, 1.0, 1.0, 1.0) == hard.ERR_ARG        # radiation not enabled
+    assert b"hard_enable_radiation" in h.L.hard_last_error(h.h)
+    st = wl.random_state((8, 8, 8), 1)
+    h.set_state(*st)
+    assert h.L.hard_set_scheme(h.h, 1) == hard.ERR_ARG                          # layout is fixed once a state exists
+    assert h.L.hard_enable_radiation(h.h) == hard.ERR_ARG
+    h.close()
