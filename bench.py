@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--scheme", default="A", choices=["A", "B"])
     ap.add_argument("--variant", default="fused", choices=["fused", "perdir"])
     ap.add_argument("--radiation", action="store_true", help="NEXT-1: carry E_rad as a sixth advected field")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: split ONE mesh into z-slabs with halo exchange (NEXT-4, strong scaling) instead of replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -178,7 +180,19 @@ def run_cuda(args):
     variant = hard.VARIANT_FUSED if args.variant == "fused" else hard.VARIANT_PERDIR
     w = wl.turbulence(n, nsteps=K, device=dev)
     cells = n ** 3
-    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing, radiation=args.radiation)
+    shard = args.shard and world > 1 and not args.radiation and variant == hard.VARIANT_FUSED
+    if shard:
+        from paper_2509_08971_b200 import sharded
+        sh = sharded.ShardedHard(w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+        h = sh.slab.h
+        slab_cells = n * n * (sh.slab.k1 - sh.slab.k0)
+        set_state = lambda: sh.set_state(w.state)
+        do_step = lambda k: sh.step(w.cfl, k)
+    else:
+        h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing, radiation=args.radiation)
+        slab_cells = cells
+        set_state = lambda: h.set_state(*w.state)
+        do_step = lambda k: h.step(w.cfl, k)
     stream = torch.cuda.current_stream()
     nfields = 6 if args.radiation else 5
     alg_bytes = ALG_BYTES_PER_CELL_STAGE * nfields / 5.0
@@ -190,11 +204,11 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing: inputs already in HBM when the timed region starts
-    h.set_state(*w.state)
+    set_state()
     if args.radiation:
         h.set_rad_energy(e_rad)
-    h.step(w.cfl, W)                       # warm-up steps (untimed)
-    h.set_state(*w.state)                  # timed steps are exactly the workload's steps 1..K
+    do_step(W)                             # warm-up steps (untimed)
+    set_state()                            # timed steps are exactly the workload's steps 1..K
     if args.radiation:
         h.set_rad_energy(e_rad)
     fp64_peak = hard.probe_fp64_peak()
@@ -207,7 +221,7 @@ def run_cuda(args):
     barrier()
     t0 = time.time()
     e0.record(stream)
-    h.step(w.cfl, K)
+    do_step(K)
     e1.record(stream)
     barrier()
     t1 = time.time()
@@ -217,7 +231,7 @@ def run_cuda(args):
     clocks = sampler.stop(t0, t1)
     t_sim, steps_done = h.time()
     ms = max_over_ranks(ms, dev)
-    value = job_throughput(cells, 2, K, ms, world)
+    value = job_throughput(cells, 2, K, ms, 1 if shard else world)
 
     # ---- roofline of the dominant kernel (the stage kernel), live CUDA-event durations
     peaks = {}
@@ -229,7 +243,7 @@ def run_cuda(args):
     hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     per_launch_ms = stage_ms / max(stage_launches, 1)
     if variant == hard.VARIANT_FUSED:
-        cell_stages_per_launch = cells                       # one launch = one RK stage over the mesh
+        cell_stages_per_launch = slab_cells                  # one launch = one RK stage over the (local) mesh
     else:
         cell_stages_per_launch = cells * 2.0 * K / max(stage_launches, 1)
     alg_gbs = cell_stages_per_launch * alg_bytes / (per_launch_ms * 1e-3) / 1e9
@@ -247,7 +261,7 @@ def run_cuda(args):
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): H2D + K steps + D2H inside the timed region
     e2e = None
-    if not args.no_e2e and not args.radiation:
+    if not args.no_e2e and not args.radiation and not shard:
         try:
             host_in = [torch.empty((n, n, n), dtype=torch.float64, pin_memory=True) for _ in range(5)]
             for a, b in zip(host_in, w.state):
@@ -282,11 +296,11 @@ def run_cuda(args):
                                   "sine-mode recipe at %d^3 (the %d^3 mesh would take hours)" % (sb, nb, n)}
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": "%s: %d^3 periodic seeded sine-mode field, CFL %.2g, %d Heun steps" % (args.workload, n, w.cfl, K),
                            "scheme": "A: WENO5-Z + HLL + Heun (PAPER.md P:151)" if args.scheme == "A" else "B: MUSCL-minmod + HLLC + SSP-RK2 (north_star fallback)",
-                           "variant": args.variant, "fields": nfields, "parallelism": "replicas x%d" % world,
+                           "variant": args.variant, "fields": nfields, "parallelism": ("z-slabs x%d (halo exchange + all-reduce max)" % world) if shard else ("replicas x%d" % world),
                            "l2": "state (%.1f GB per buffer) is far larger than the 126 MB L2; no flush needed" % (5 * cells * 8 / 1e9),
                            "sim_time": t_sim, "steps_done": steps_done},
                 "roofline": roofline, "roofline_hbm": roofline_hbm, "e2e": e2e, "cpu_baseline": cpu_baseline,

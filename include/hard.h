@@ -96,6 +96,28 @@ int hard_get_rad_energy(hard_ctx*, double* e_rad);
  * conserved exactly.  Needs hard_enable_radiation.  kappa >= 0, the other parameters > 0 (any unit system). */
 int hard_set_source(hard_ctx*, double kappa, double c_light, double a_rad, double cv);
 
+/* ---- NEXT-4 (SURVEY §8(e),(f)): z-slab sharding over several GPUs, one hard_ctx per rank -------------------
+ * Each rank creates its context with its own nz (>= g planes) and tells which z faces border a neighbour rank
+ * (their ghost planes are then filled by the halo exchange instead of the boundary condition).  A step is driven
+ * phase by phase so that the caller can exchange halos in between (paper_2509_08971_b200/sharded.py does it with
+ * NCCL send/recv and one all-reduce(MAX) of lambda per step, all stream-ordered, no host synchronisation):
+ *   exchange halos of buffer 0; GHOST_U; STAGE1; exchange halos of buffer 1; GHOST_U1; STAGE2;
+ *   all-reduce(MAX) the double at hard_lambda_ptr(next = 1); END.
+ * After hard_set_state the double at hard_lambda_ptr(next = 0) must be all-reduced likewise. */
+enum { HARD_PHASE_GHOST_U = 0, HARD_PHASE_STAGE1 = 1, HARD_PHASE_GHOST_U1 = 2, HARD_PHASE_STAGE2 = 3, HARD_PHASE_END = 4 };
+int hard_set_slab(hard_ctx*, int lower_neighbor, int upper_neighbor);
+/* Doubles in one halo buffer: g * nx * ny * fields, laid out [field][plane][y][x]. */
+size_t hard_halo_doubles(const hard_ctx*);
+/* buffer: 0 = U, 1 = U1.  pack: side 0 / 1 = the g lowest / highest interior planes (for the lower / upper
+ * neighbour).  unpack: side 0 / 1 = into the low / high ghost planes.  dev_buf is device memory. */
+int hard_halo_pack(hard_ctx*, int buffer, int side, double* dev_buf);
+int hard_halo_unpack(hard_ctx*, int buffer, int side, const double* dev_buf);
+/* One phase of a step (HARD_PHASE_*); dt > 0 fixes the step, else dt = cfl / lambda.  Fused variant only. */
+int hard_substep(hard_ctx*, double cfl, double dt, int phase);
+/* Device address of lambda_max of the current state (next = 0) or of the state the running step produces
+ * (next = 1), as a non-negative double, for an in-place all-reduce(MAX) across ranks. */
+int hard_lambda_ptr(hard_ctx*, int next, double** dev_ptr);
+
 /* HARD_VARIANT_*; may be switched at any time between steps (same state buffers). */
 int hard_set_variant(hard_ctx*, int variant);
 

@@ -31,6 +31,7 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct hard_ctx {
   GridDesc g;
   int scheme = HARD_SCHEME_WENO5Z_HLL, variant = HARD_VARIANT_FUSED;
+  int zskip = 0;                    // NEXT-4: z ghost faces that a neighbour rank fills (hard_set_slab)
   bool src_on = false;              // NEXT-3: heating/cooling source after every step (hard_set_source)
   SourceParams src{};
   int nf = 5;                       // 6 with the advected radiation energy density (hard_enable_radiation)
@@ -82,6 +83,7 @@ void compute_layout(hard_ctx* c) {
   GridDesc& g = c->g;
   g.g = (c->scheme == HARD_SCHEME_WENO5Z_HLL) ? 3 : 2;
   g.nf = c->nf;
+  g.zskip = c->zskip;
   for (int a = 0; a < 3; ++a) g.act[a] = g.n[a] > 1;
   // x: ghost width g on the left, so that a tile's TMA box (which starts g cells left of the tile)
   // starts at padded x-coordinate i0, a multiple of 16 doubles: the box start must be 16-byte
@@ -432,6 +434,58 @@ int hard_set_source(hard_ctx* c, double kappa, double c_light, double a_rad, dou
   if (!(kappa >= 0.0 && c_light > 0.0 && a_rad > 0.0 && cv > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_source: bad parameter");
   c->src_on = true;
   c->src.kappa = kappa; c->src.c_light = c_light; c->src.a_rad = a_rad; c->src.cv = cv;
+  return HARD_OK;
+}
+
+int hard_set_slab(hard_ctx* c, int lower_neighbor, int upper_neighbor) {
+  if (!c) return HARD_ERR_ARG;
+  if (!c->g.act[2]) return fail(c, HARD_ERR_ARG, "hard_set_slab: the z direction is inactive");
+  c->zskip = (lower_neighbor ? 1 : 0) | (upper_neighbor ? 2 : 0);
+  c->g.zskip = c->zskip;
+  return HARD_OK;
+}
+
+size_t hard_halo_doubles(const hard_ctx* c) {
+  return c ? (size_t)c->g.g * c->g.n[0] * c->g.n[1] * c->nf : 0;
+}
+
+static int halo_copy(hard_ctx* c, int buffer, int side, double* buf, int unpack) {
+  if (!c || !buf || (buffer != 0 && buffer != 1) || (side != 0 && side != 1)) return fail(c, HARD_ERR_ARG, "hard_halo_*: bad argument");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
+  if (!c->g.act[2] || c->g.n[2] < c->g.g) return fail(c, HARD_ERR_ARG, "hard_halo_*: a slab needs at least g z-planes");
+  const long long total = (long long)hard_halo_doubles(c);
+  halo_copy_kernel<<<small_grid(c, total), 256, 0, c->stream>>>(buffer ? c->U1 : c->U, buf, c->g, side, unpack);
+  return after_launch(c, "halo_copy_kernel");
+}
+int hard_halo_pack(hard_ctx* c, int buffer, int side, double* dev_buf) { return halo_copy(c, buffer, side, dev_buf, 0); }
+int hard_halo_unpack(hard_ctx* c, int buffer, int side, const double* dev_buf) {
+  return halo_copy(c, buffer, side, const_cast<double*>(dev_buf), 1);
+}
+
+int hard_substep(hard_ctx* c, double cfl, double dt, int phase) {
+  if (!c || !((dt > 0.0) || (cfl > 0.0))) return fail(c, HARD_ERR_ARG, "hard_substep: cfl > 0 or dt > 0 required");
+  if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
+  if (c->variant != HARD_VARIANT_FUSED) return fail(c, HARD_ERR_ARG, "hard_substep: fused variant only");
+  int rc = ensure_ready(c);
+  if (rc) return rc;
+  const double dtf = dt > 0.0 ? dt : 0.0, cf = dt > 0.0 ? 1.0 : cfl;
+  switch (phase) {
+    case HARD_PHASE_GHOST_U:  return launch_ghost(c, c->U, 1, cf, dtf);
+    case HARD_PHASE_STAGE1:   return launch_stage(c, c->tmU, c->U, nullptr, c->U1, MODE_STAGE1, 7, 0, cf, dtf);
+    case HARD_PHASE_GHOST_U1: return launch_ghost(c, c->U1, 0, cf, dtf);
+    case HARD_PHASE_STAGE2:
+      if ((rc = launch_stage(c, c->tmU1, c->U1, c->U, c->U, MODE_STAGE2, 7, 0, cf, dtf))) return rc;
+      return c->src_on ? launch_source(c, cf, dtf) : HARD_OK;
+    case HARD_PHASE_END:      c->steps_enq++; return HARD_OK;
+    default: return fail(c, HARD_ERR_ARG, "hard_substep: unknown phase");
+  }
+}
+
+int hard_lambda_ptr(hard_ctx* c, int next, double** dev_ptr) {
+  if (!c || !dev_ptr) return HARD_ERR_ARG;
+  int rc = ensure_ready(c);
+  if (rc) return rc;
+  *dev_ptr = reinterpret_cast<double*>(&c->sc->lam_bits[(c->steps_enq & 1) ^ (next ? 1 : 0)]);
   return HARD_OK;
 }
 

@@ -25,6 +25,7 @@ struct GridDesc {
   int bc;                   // 0 periodic, 1 outflow, 2 reflecting
   int g;                    // ghost width of the scheme
   int nf;                   // fields per state: 5, or 6 with the advected radiation energy density (NEXT-1)
+  int zskip;                // NEXT-4 z-slab sharding: bit 0 / 1 = low / high z ghosts come from a neighbour rank
 };
 
 // Device-resident scalars: nothing returns to the host inside hard_step.
@@ -94,6 +95,7 @@ __global__ void ghost_fill_kernel(double* __restrict__ U, GridDesc g, DevScalars
       c[1] = (int)(r % ny); m = (int)(r / ny);
     }
     const int n = g.n[d];
+    if (d == 2 && ((m < G) ? (g.zskip & 1) : (g.zskip & 2))) continue;   // filled by the halo exchange
     int dst, src;
     if (m < G) {                                    // low side, layer m+1
       dst = -(m + 1);
@@ -187,6 +189,28 @@ __global__ void axpy_kernel(const double* __restrict__ Un, const double* __restr
       if (!stage2) out[q] = fma(dt, R[q], Un[q]);
       else out[q] = 0.5 * Un[q] + 0.5 * fma(dt, R[q], U1[q]);
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------- NEXT-4: z-slab halos
+// Pack the g lowest / highest interior z-planes of all fields into a contiguous buffer [nf][g][ny][nx]
+// (to be sent to the lower / upper neighbour rank), or unpack such a buffer into the low / high z ghost
+// planes.  side: 0 = low, 1 = high.  Interior x-y only: the stencils never read edges or corners.
+__global__ void halo_copy_kernel(double* __restrict__ U, double* __restrict__ buf, GridDesc g, int side, int unpack) {
+  const int G = g.g;
+  const long long plane = (long long)g.n[0] * g.n[1], per_field = plane * G, total = per_field * g.nf;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int f = (int)(idx / per_field);
+    long long r = idx - f * per_field;
+    const int m = (int)(r / plane);
+    r -= m * plane;
+    const int j = (int)(r / g.n[0]), i = (int)(r - (long long)j * g.n[0]);
+    int k;
+    if (!unpack) k = side ? g.n[2] - G + m : m;              // interior planes to send
+    else         k = side ? g.n[2] + m : m - G;              // ghost planes to fill
+    const long long p = f * g.fstride + cell_addr(g, i, j, k);
+    if (unpack) U[p] = buf[idx]; else buf[idx] = U[p];
   }
 }
 

@@ -23,7 +23,8 @@ EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard
            "hard_set_spacing", "hard_set_scheme", "hard_set_variant", "hard_set_stream", "hard_workspace_bytes",
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
            "hard_stage_time", "hard_probe_fp64_peak", "hard_enable_radiation", "hard_set_rad_energy",
-           "hard_get_rad_energy", "hard_set_source"]
+           "hard_get_rad_energy", "hard_set_source", "hard_set_slab", "hard_halo_doubles", "hard_halo_pack",
+           "hard_halo_unpack", "hard_substep", "hard_lambda_ptr"]
 
 _lib = None
 
@@ -63,6 +64,13 @@ def lib():
     L.hard_set_rad_energy.argtypes = [vp, dp]
     L.hard_get_rad_energy.argtypes = [vp, dp]
     L.hard_set_source.argtypes = [vp, c_dbl, c_dbl, c_dbl, c_dbl]
+    L.hard_set_slab.argtypes = [vp, c_int, c_int]
+    L.hard_halo_doubles.restype = ctypes.c_size_t
+    L.hard_halo_doubles.argtypes = [vp]
+    L.hard_halo_pack.argtypes = [vp, c_int, c_int, dp]
+    L.hard_halo_unpack.argtypes = [vp, c_int, c_int, dp]
+    L.hard_substep.argtypes = [vp, c_dbl, c_dbl, c_int]
+    L.hard_lambda_ptr.argtypes = [vp, c_int, ctypes.POINTER(ctypes.c_void_p)]
     L.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(c_dbl), ctypes.POINTER(c_dbl)]
     _lib = L
     return L
@@ -156,6 +164,27 @@ class Hard:
         return v.value
 
     # ---- extensions
+    # ---- NEXT-4: z-slab sharding primitives (see sharded.py)
+    def set_slab(self, lower, upper):
+        self._chk(self.L.hard_set_slab(self.h, int(lower), int(upper)))
+
+    def halo_doubles(self):
+        return int(self.L.hard_halo_doubles(self.h))
+
+    def halo_pack(self, buffer, side, buf):
+        self._chk(self.L.hard_halo_pack(self.h, buffer, side, _ptr(buf)))
+
+    def halo_unpack(self, buffer, side, buf):
+        self._chk(self.L.hard_halo_unpack(self.h, buffer, side, _ptr(buf)))
+
+    def substep(self, phase, cfl=0.0, dt=0.0):
+        self._chk(self.L.hard_substep(self.h, float(cfl), float(dt), int(phase)))
+
+    def lambda_ptr(self, nxt):
+        p = ctypes.c_void_p()
+        self._chk(self.L.hard_lambda_ptr(self.h, int(nxt), ctypes.byref(p)))
+        return p.value
+
     def set_source(self, kappa, c_light, a_rad, cv):
         self._chk(self.L.hard_set_source(self.h, float(kappa), float(c_light), float(a_rad), float(cv)))
 
