@@ -129,3 +129,27 @@ def test_argument_errors():
     assert h.L.hard_set_scheme(h.h, 1) == hard.ERR_ARG                          # layout is fixed once a state exists
     assert h.L.hard_enable_radiation(h.h) == hard.ERR_ARG
     h.close()
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+@pytest.mark.parametrize("n,bc", [((37, 21, 19), wl.BC_PERIODIC), ((30, 17, 1), wl.BC_OUTFLOW), ((45, 1, 1), wl.BC_REFLECT)])
+def test_nan_poisoned_workspace(scheme, n, bc):
+    """Everything the kernels may legitimately read is written by set_state / ghost fill / the stages: poison the
+    whole workspace (ghost edges and corners, pitch padding, U1, the residual buffer) with NaN first; a single read
+    of a never-written location by a valid cell would surface as NaN in the result (compute-sanitizer is closed on
+    this pool, so this and the ragged-shape parity cases are the bounds evidence)."""
+    import torch
+    w = wl.Workload("r", n, 1.4, bc, (0.1, 0.07, 0.13), 0.4, nsteps=3, state=wl.random_state(n, 8))
+    ref, _ = _oracle_run(w, scheme, 3)
+    for variant in (hard.VARIANT_FUSED, hard.VARIANT_PERDIR):
+        h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing)
+        torch.cuda.synchronize()
+        base = (h.ws.data_ptr() + 255) // 256 * 256 - h.ws.data_ptr()
+        body = h.ws[base + 256: base + (h.workspace_bytes() // 8) * 8].view(torch.float64)   # after the scalar block
+        body.fill_(float("nan"))
+        h.set_state(*w.state)
+        h.step(w.cfl, 3)
+        out = h.get_state()
+        assert all(np.isfinite(a).all() for a in out)
+        assert max(field_errors(out, ref)) <= 1e-11
+        h.close()
