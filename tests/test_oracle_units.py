@@ -42,10 +42,9 @@ def _cell_avg_poly(coef, i):
     return P(i + 0.5) - P(i - 0.5)
 
 
-def test_wenoz_linear_weights_are_fifth_order():
-    # uniform second differences => beta0 = beta2 is not implied, so use data where tau = 0:
-    # any polynomial of degree <= 2 has b0 == b2?  No — instead check the documented property:
-    # for degree <= 2 all three candidates are exact, so any convex weights give the exact value.
+def test_wenoz_exact_for_polynomials_up_to_degree_two():
+    # every one of the three candidate stencils reproduces a polynomial of degree <= 2 exactly from its cell
+    # averages, so any convex combination (whatever the nonlinear weights) gives the exact face value
     for coef in ([1.0], [0.3, -2.0], [1.0, 0.5, -0.7]):
         avg = [_cell_avg_poly(coef, i) for i in range(-2, 3)]
         exact_face = np.polynomial.Polynomial(coef)(0.5)
