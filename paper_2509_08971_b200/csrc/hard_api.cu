@@ -85,11 +85,10 @@ void compute_layout(hard_ctx* c) {
   g.nf = c->nf;
   g.zskip = c->zskip;
   for (int a = 0; a < 3; ++a) g.act[a] = g.n[a] > 1;
-  // x: ghost width g on the left, so that a tile's TMA box (which starts g cells left of the tile)
-  // starts at padded x-coordinate i0, a multiple of 16 doubles: the box start must be 16-byte
-  // aligned (measured: an odd fp64 start coordinate raises "illegal instruction" on sm_100a) and
-  // every box row then starts on a 128-B line.  Row pitch: a multiple of 16 doubles (TMA strides
-  // must be multiples of 16 B).
+  // x: ghost width g on the left, so that a tile's TMA box (which starts g cells left of the 14-cell tile)
+  // starts at padded x-coordinate 14 * tile, an EVEN coordinate: the innermost start coordinate of an fp64
+  // box must be 16-byte aligned (measured: an odd start raises "illegal instruction" on sm_100a).
+  // Row pitch: a multiple of 16 doubles (TMA strides must be multiples of 16 B; rows start on 128-B lines).
   g.off[0] = g.g;   // also when x is inactive (the columns stay zero and are never read by a valid cell)
   g.off[1] = g.act[1] ? g.g : 0;
   g.off[2] = g.act[2] ? g.g : 0;
