@@ -153,3 +153,17 @@ def test_nan_poisoned_workspace(scheme, n, bc):
         assert all(np.isfinite(a).all() for a in out)
         assert max(field_errors(out, ref)) <= 1e-11
         h.close()
+
+
+def test_zero_steps_is_a_no_op_and_get_set_roundtrip_is_exact():
+    n = (19, 14, 11)
+    st = wl.random_state(n, 4)
+    h = hard.Hard(*n, 1.4, wl.BC_OUTFLOW, spacing=(0.1, 0.1, 0.1))
+    h.set_state(*st)
+    h.step(0.4, 0)
+    h.step_dt(1e-3, 0)
+    out = h.get_state()
+    for a, b in zip(out, st):
+        assert np.array_equal(a, b)             # set/get copy the interior bit for bit
+    assert h.time() == (0.0, 0)
+    h.close()
