@@ -152,15 +152,9 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     const double E = W[4] * inv_gm1 + 0.5 * W[0] * (W[1] * W[1] + (W[2] * W[2] + W[3] * W[3]));
     const double UK[5] = { W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E };
     const double FK[5] = { UK[1], UK[1] * W[1] + W[4], UK[1] * W[2], UK[1] * W[3], (E + W[4]) * W[1] };
-    if (supL || supR) {
-#pragma unroll
-      for (int m = 0; m < 5; ++m) F[m] = FK[m];
-      return;
-    }
-    if (Ss == 0.0) {
-      F[0] = 0.0; F[1] = pbar; F[2] = 0.0; F[3] = 0.0; F[4] = 0.0;
-      return;
-    }
+    // Branch-free tail: S* = 0 needs no special case here (the formula gives (0, pbar, 0, 0, 0) exactly:
+    // every term carries the factor S* except SK pbar / SK), and the supersonic cases select F_K.
+    const bool sup = supL || supR;
     const double inv = fast_rcp(SK - Ss);
     const double sp = SK * pbar;
 #pragma unroll
@@ -168,7 +162,7 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
       double t = Ss * (SK * UK[m] - FK[m]);
       if (m == 1) t += sp;
       if (m == 4) t = fma(sp, Ss, t);
-      F[m] = t * inv;
+      F[m] = sup ? FK[m] : t * inv;
     }
   }
 }
