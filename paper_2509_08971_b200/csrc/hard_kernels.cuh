@@ -1,8 +1,11 @@
-// hard_kernels.cuh — CUDA kernels of the hot path for sm_100a (SURVEY.md §8(a) rows a1..a8):
-//   ghost_fill_kernel   a1  ghost-cell fill, all faces of active directions, one launch
-//   stage_kernel<S>     a2..a6 (+a7 fused in stage 2): TMA-staged x-y tile marched along z
-//   cfl_kernel          a7  standalone max-wavespeed reduction (set_state, per-direction variant)
-//   axpy_kernel         a6  RK combination of the per-direction variant (a8)
+// hard_kernels.cuh — CUDA kernels of the hot path for sm_100a (SURVEY.md §8(a) rows a1..a8, §8(f) NEXT rows):
+//   ghost_fill_kernel    a1  ghost-cell fill (periodic / outflow / reflecting), all faces, one launch
+//   stage_kernel<S, NF>  a2..a6 (+a7 fused in stage 2): TMA-staged 14x16 x-y tile marched along z;
+//                        NF = 6 carries the advected radiation energy density (NEXT-1, Rusanov flux)
+//   cfl_kernel           a7  standalone max-wavespeed reduction (set_state, per-direction variant)
+//   axpy_kernel          a6  RK combination of the per-direction variant (a8)
+//   source_kernel        NEXT-3  pointwise heating / cooling source (backward Euler) + the step's CFL reduction
+//   halo_copy_kernel     NEXT-4  pack / unpack z-slab halo planes for the exchange between ranks
 // The stage kernel also serves the per-direction comparison variant (a8): dirmask selects one
 // direction and MODE_RESID read-modify-writes a residual array instead of applying the RK update.
 #pragma once
