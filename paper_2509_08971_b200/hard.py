@@ -35,8 +35,12 @@ def lib():
     if _lib is not None:
         return _lib
     if not os.path.exists(LIB_PATH):
-        raise RuntimeError("libhard_b200.so is not built: run `python -m paper_2509_08971_b200.build` "
-                           "(there is no CPU fallback)")
+        try:                                   # compile it (nvcc, sm_100a); this is a build step, not a fallback
+            from . import build as _build
+            _build.build()
+        except Exception as ex:
+            raise RuntimeError("libhard_b200.so is not built and could not be compiled (%s): run "
+                               "`python -m paper_2509_08971_b200.build` (there is no CPU fallback)" % ex)
     L = ctypes.CDLL(LIB_PATH)
     vp, dp, c_int, c_dbl = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_double
     L.hard_create.restype = vp
