@@ -263,6 +263,12 @@ def run_cuda(args):
     e2e = None
     if not args.no_e2e and not args.radiation and not shard:
         try:
+            import psutil
+            need = 2 * 5 * cells * 8                       # pinned input + output copies of the state
+            avail = psutil.virtual_memory().available / max(world, 1)
+            if avail < 1.3 * need:
+                raise MemoryError("host memory: %.0f GB available per rank, %.0f GB of pinned buffers needed"
+                                  % (avail / 1e9, need / 1e9))
             host_in = [torch.empty((n, n, n), dtype=torch.float64, pin_memory=True) for _ in range(5)]
             for a, b in zip(host_in, w.state):
                 a.copy_(b)
