@@ -51,6 +51,12 @@ struct hard_ctx {
   std::string err;
   bool profiling = false;
   bool debug_sync = false;            // HARD_DEBUG_SYNC=1: synchronise and check after every launch
+  // CUDA graph of two consecutive steps (even + odd lambda slot), replayed by hard_step* on capturable streams
+  cudaGraphExec_t gexec = nullptr;
+  double g_cfl = 0.0, g_dt = 0.0;
+  int g_sig = -1;                   // variant / source / stream signature the graph was captured for
+  cudaStream_t g_stream = nullptr;
+  bool graphs_ok = true;            // cleared when the bound stream cannot be captured (legacy default stream)
   std::vector<cudaEvent_t> ev;      // start/stop pairs around stage kernels
   size_t ev_used = 0;
 };
@@ -281,28 +287,78 @@ int perdir_residual(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, doub
   return HARD_OK;
 }
 
+int enqueue_one_step(hard_ctx* c, double cfl, double dt_fixed) {
+  int rc;
+  if ((rc = launch_ghost(c, c->U, 1, cfl, dt_fixed))) return rc;
+  if (c->variant == HARD_VARIANT_FUSED) {
+    if ((rc = launch_stage(c, c->tmU, c->U, nullptr, c->U1, MODE_STAGE1, 7, 0, cfl, dt_fixed))) return rc;
+    if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
+    if ((rc = launch_stage(c, c->tmU1, c->U1, c->U, c->U, MODE_STAGE2, 7, 0, cfl, dt_fixed))) return rc;
+    if (c->src_on && (rc = launch_source(c, cfl, dt_fixed))) return rc;
+  } else {
+    if ((rc = perdir_residual(c, c->tmU, c->U, cfl, dt_fixed))) return rc;
+    if ((rc = launch_axpy(c, 0, cfl, dt_fixed))) return rc;
+    if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
+    if ((rc = perdir_residual(c, c->tmU1, c->U1, cfl, dt_fixed))) return rc;
+    if ((rc = launch_axpy(c, 1, cfl, dt_fixed))) return rc;
+    if (c->src_on) { if ((rc = launch_source(c, cfl, dt_fixed))) return rc; }
+    else if ((rc = launch_cfl(c, c->U, (int)((c->steps_enq & 1) ^ 1)))) return rc;
+  }
+  c->steps_enq++;
+  return HARD_OK;
+}
+
+// Launch-bound meshes (the 1-D configs: ~10^3 cells, ~10^4 steps): replay a captured graph of two steps.  dt and
+// lambda live on the device, so the graph needs no host value; the pair covers both lambda ping-pong slots.
+// Only on capturable streams (not the legacy default stream), never while stage timing is on.
+bool ensure_graph(hard_ctx* c, double cfl, double dt_fixed) {
+  static const bool disabled = getenv("HARD_NO_GRAPH") != nullptr;
+  if (disabled || !c->graphs_ok || c->profiling || c->debug_sync || (c->steps_enq & 1)) return false;
+  const int sig = c->variant * 4 + (c->src_on ? 2 : 0) + 1;
+  if (c->gexec && c->g_cfl == cfl && c->g_dt == dt_fixed && c->g_sig == sig && c->g_stream == c->stream) return true;
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+  if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    c->graphs_ok = false;
+    return false;
+  }
+  const long long enq0 = c->steps_enq, l0 = c->launches;
+  int rc = enqueue_one_step(c, cfl, dt_fixed);
+  if (!rc) rc = enqueue_one_step(c, cfl, dt_fixed);
+  c->steps_enq = enq0;                                   // nothing ran: capture only
+  c->launches = l0;
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+  if (rc || e != cudaSuccess || !graph) { cudaGetLastError(); c->graphs_ok = false; if (graph) cudaGraphDestroy(graph); return false; }
+  e = cudaGraphInstantiate(&c->gexec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { cudaGetLastError(); c->gexec = nullptr; c->graphs_ok = false; return false; }
+  c->g_cfl = cfl; c->g_dt = dt_fixed; c->g_sig = sig; c->g_stream = c->stream;
+  return true;
+}
+
 int do_steps(hard_ctx* c, double cfl, double dt_fixed, int nsteps) {
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
   int rc = ensure_ready(c);
   if (rc) return rc;
-  for (int s = 0; s < nsteps; ++s) {
-    if ((rc = launch_ghost(c, c->U, 1, cfl, dt_fixed))) return rc;
-    if (c->variant == HARD_VARIANT_FUSED) {
-      if ((rc = launch_stage(c, c->tmU, c->U, nullptr, c->U1, MODE_STAGE1, 7, 0, cfl, dt_fixed))) return rc;
-      if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
-      if ((rc = launch_stage(c, c->tmU1, c->U1, c->U, c->U, MODE_STAGE2, 7, 0, cfl, dt_fixed))) return rc;
-      if (c->src_on && (rc = launch_source(c, cfl, dt_fixed))) return rc;
-    } else {
-      if ((rc = perdir_residual(c, c->tmU, c->U, cfl, dt_fixed))) return rc;
-      if ((rc = launch_axpy(c, 0, cfl, dt_fixed))) return rc;
-      if ((rc = launch_ghost(c, c->U1, 0, cfl, dt_fixed))) return rc;
-      if ((rc = perdir_residual(c, c->tmU1, c->U1, cfl, dt_fixed))) return rc;
-      if ((rc = launch_axpy(c, 1, cfl, dt_fixed))) return rc;
-      if (c->src_on) { if ((rc = launch_source(c, cfl, dt_fixed))) return rc; }
-      else if ((rc = launch_cfl(c, c->U, (int)((c->steps_enq & 1) ^ 1)))) return rc;
+  int left = nsteps;
+  if (left >= 8 && c->stream != 0 && c->variant == HARD_VARIANT_FUSED) {
+    if (c->steps_enq & 1) {                              // the captured pair starts on an even step
+      if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return rc;
+      --left;
     }
-    c->steps_enq++;
+    if (ensure_graph(c, cfl, dt_fixed)) {
+      const long long per_pair = 8 + (c->src_on ? 2 : 0);
+      while (left >= 2) {
+        CK(cudaGraphLaunch(c->gexec, c->stream));
+        c->steps_enq += 2;
+        c->launches += per_pair;
+        left -= 2;
+      }
+    }
   }
+  for (; left > 0; --left)
+    if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return rc;
   return HARD_OK;
 }
 
@@ -373,6 +429,7 @@ int hard_destroy(hard_ctx* c) {
   if (!c) return HARD_ERR_ARG;
   cudaStreamSynchronize(c->stream);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->gexec) cudaGraphExecDestroy(c->gexec);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
   delete c;
   return HARD_OK;

@@ -167,3 +167,32 @@ def test_zero_steps_is_a_no_op_and_get_set_roundtrip_is_exact():
         assert np.array_equal(a, b)             # set/get copy the interior bit for bit
     assert h.time() == (0.0, 0)
     h.close()
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_graph_replay_on_a_capturable_stream_matches_direct_launches(scheme):
+    """hard_step with >= 8 steps on a non-default stream replays a captured two-step CUDA graph (launch-bound 1-D
+    configs); the result must equal the directly launched run bit for bit, for even and odd step counts."""
+    import torch
+    w = wl.sod(1000)
+    ref = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)     # default stream: direct launches
+    ref.set_state(*w.state)
+    ref.step(w.cfl, 3)
+    ref.step(w.cfl, 25)
+    ref.step_dt(1e-5, 9)
+    exp, t_exp = ref.get_state(), ref.time()
+    n_direct = ref.launch_count()
+    ref.close()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+        h.set_state(*w.state)
+        h.step(w.cfl, 3)                   # direct (fewer than 8), leaves an odd step count
+        h.step(w.cfl, 25)                  # one direct step to even out + 12 graph replays
+        h.step_dt(1e-5, 9)                 # new graph (fixed dt): 4 replays + 1 direct
+        out, t_out = h.get_state(), h.time()
+        assert h.launch_count() == n_direct
+    for a, b in zip(out, exp):
+        assert np.array_equal(a, b)
+    assert t_out == t_exp
+    h.close()
