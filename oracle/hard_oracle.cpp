@@ -354,10 +354,9 @@ void apply_source(Ctx* c, double dt) {
           if (gx > 0.0) hi = x; else lo = x;
           double dg = 1.0 + beta * (1.0 + 4.0 * c->src_a * T2 * T / rcv);
           double xn = x - gx / dg;
-          if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);            // Newton left the bracket: bisect
-          double dx = std::fabs(xn - x);
+          if (std::fabs(xn - x) <= 1e-15 * std::fabs(xn)) { x = xn; break; }   // converged (also onto a bracket end)
+          if (!(xn >= lo && xn <= hi)) xn = 0.5 * (lo + hi);           // Newton left the bracket: bisect
           x = xn;
-          if (dx <= 1e-15 * std::fabs(x)) break;
         }
         c->U[4][p] = x + ke;
         c->U[5][p] = Etot - x;

@@ -246,20 +246,19 @@ __global__ void source_kernel(double* __restrict__ U, GridDesc g, DevScalars* sc
     for (int f = 0; f < 5; ++f) Uc[f] = U[f * g.fstride + p];
     const double Er = U[5 * g.fstride + p];
     const double rho = Uc[0];
-    const double ke = 0.5 * (Uc[1] * Uc[1] + Uc[2] * Uc[2] + Uc[3] * Uc[3]) / rho;
+    const double ke = 0.5 * (Uc[1] * Uc[1] + Uc[2] * Uc[2] + Uc[3] * Uc[3]) * fast_rcp(rho);
     const double e = Uc[4] - ke, Etot = e + Er;
-    const double beta = dt * sp.c_light * sp.kappa * rho, rcv = rho * sp.cv, inv_rcv = 1.0 / rcv;
+    const double beta = dt * sp.c_light * sp.kappa * rho, rcv = rho * sp.cv, inv_rcv = fast_rcp(rcv);
     double lo = 0.0, hi = Etot, x = e < 0.0 ? 0.0 : (e > Etot ? Etot : e);
     for (int it = 0; it < 200; ++it) {
       const double T = x * inv_rcv, T2 = T * T, T4 = T2 * T2;
       const double gx = (x - e) - beta * ((Etot - x) - sp.a_rad * T4);
       if (gx > 0.0) hi = x; else lo = x;
       const double dg = 1.0 + beta * (1.0 + 4.0 * sp.a_rad * T2 * T * inv_rcv);
-      double xn = x - gx / dg;
-      if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);
-      const double dx = fabs(xn - x);
+      double xn = fma(-gx, fast_rcp(dg), x);                   // dg >= 1: normal
+      if (fabs(xn - x) <= 1e-15 * fabs(xn)) { x = xn; break; }  // converged (also onto a bracket end)
+      if (!(xn >= lo && xn <= hi)) xn = 0.5 * (lo + hi);       // Newton left the bracket: bisect
       x = xn;
-      if (dx <= 1e-15 * fabs(x)) break;
     }
     Uc[4] = x + ke;
     U[4 * g.fstride + p] = Uc[4];
