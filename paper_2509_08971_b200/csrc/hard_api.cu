@@ -48,6 +48,7 @@ struct hard_ctx {
   long long launches = 0;
   int Lz = 0;
   int sm_count = 148;
+  int device = 0;                   // the CUDA device the context was created on
   std::string err;
   bool profiling = false;
   bool debug_sync = false;            // HARD_DEBUG_SYNC=1: synchronise and check after every launch
@@ -62,6 +63,15 @@ struct hard_ctx {
 };
 
 namespace {
+
+// Entry points run on the context's device whatever the caller's current device is.
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(const hard_ctx* c) {
+    if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) cudaSetDevice(c->device); else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 int fail(hard_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg;
@@ -420,12 +430,14 @@ hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc) {
   c->g.gamma = gamma;
   c->g.bc = bc;
   c->sm_count = prop.multiProcessorCount;
+  c->device = dev;
   { const char* d = getenv("HARD_DEBUG_SYNC"); c->debug_sync = d && d[0] == '1'; }
   compute_layout(c);
   return c;
 }
 
 int hard_destroy(hard_ctx* c) {
+  DeviceGuard dg__(c);
   if (!c) return HARD_ERR_ARG;
   cudaStreamSynchronize(c->stream);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -440,6 +452,7 @@ const char* hard_last_error(const hard_ctx* c) { return c ? c->err.c_str() : g_c
 long long hard_launch_count(const hard_ctx* c) { return c ? c->launches : -1; }
 
 int hard_set_spacing(hard_ctx* c, double dx, double dy, double dz) {
+  DeviceGuard dg__(c);
   if (!c || !(dx > 0.0 && dy > 0.0 && dz > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_spacing: spacings must be > 0");
   c->g.inv_d[0] = 1.0 / dx; c->g.inv_d[1] = 1.0 / dy; c->g.inv_d[2] = 1.0 / dz;
   if (c->have_state) {
@@ -468,6 +481,7 @@ int hard_enable_radiation(hard_ctx* c) {
 }
 
 int hard_set_rad_energy(hard_ctx* c, const double* er) {
+  DeviceGuard dg__(c);
   if (!c || !er) return fail(c, HARD_ERR_ARG, "hard_set_rad_energy: null pointer");
   if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_set_rad_energy: call hard_enable_radiation first");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
@@ -475,6 +489,7 @@ int hard_set_rad_energy(hard_ctx* c, const double* er) {
 }
 
 int hard_get_rad_energy(hard_ctx* c, double* er) {
+  DeviceGuard dg__(c);
   if (!c || !er) return fail(c, HARD_ERR_ARG, "hard_get_rad_energy: null pointer");
   if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_get_rad_energy: call hard_enable_radiation first");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
@@ -506,6 +521,7 @@ size_t hard_halo_doubles(const hard_ctx* c) {
 }
 
 static int halo_copy(hard_ctx* c, int buffer, int side, double* buf, int unpack) {
+  DeviceGuard dg__(c);
   if (!c || !buf || (buffer != 0 && buffer != 1) || (side != 0 && side != 1)) return fail(c, HARD_ERR_ARG, "hard_halo_*: bad argument");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
   if (!c->g.act[2] || c->g.n[2] < c->g.g) return fail(c, HARD_ERR_ARG, "hard_halo_*: a slab needs at least g z-planes");
@@ -519,6 +535,7 @@ int hard_halo_unpack(hard_ctx* c, int buffer, int side, const double* dev_buf) {
 }
 
 int hard_substep(hard_ctx* c, double cfl, double dt, int phase) {
+  DeviceGuard dg__(c);
   if (!c || !((dt > 0.0) || (cfl > 0.0))) return fail(c, HARD_ERR_ARG, "hard_substep: cfl > 0 or dt > 0 required");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state: call hard_set_state first");
   if (c->variant != HARD_VARIANT_FUSED) return fail(c, HARD_ERR_ARG, "hard_substep: fused variant only");
@@ -538,6 +555,7 @@ int hard_substep(hard_ctx* c, double cfl, double dt, int phase) {
 }
 
 int hard_lambda_ptr(hard_ctx* c, int next, double** dev_ptr) {
+  DeviceGuard dg__(c);
   if (!c || !dev_ptr) return HARD_ERR_ARG;
   int rc = ensure_ready(c);
   if (rc) return rc;
@@ -553,6 +571,7 @@ int hard_set_variant(hard_ctx* c, int variant) {
 }
 
 int hard_set_stream(hard_ctx* c, void* s) {
+  DeviceGuard dg__(c);
   if (!c) return HARD_ERR_ARG;
   CK(cudaStreamSynchronize(c->stream));
   c->stream = (cudaStream_t)s;
@@ -565,6 +584,7 @@ size_t hard_workspace_bytes(const hard_ctx* c) {
 }
 
 int hard_bind_workspace(hard_ctx* c, void* dev, size_t bytes) {
+  DeviceGuard dg__(c);
   if (!c || !dev) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: null");
   if (c->ws) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: a workspace is already bound");
   if (bytes < hard_workspace_bytes(c) || ((uintptr_t)dev & 255)) return fail(c, HARD_ERR_ARG, "hard_bind_workspace: too small or not 256-B aligned");
@@ -580,6 +600,7 @@ int hard_bind_workspace(hard_ctx* c, void* dev, size_t bytes) {
 }
 
 int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const double* my, const double* mz, const double* E) {
+  DeviceGuard dg__(c);
   if (!c || !rho || !mx || !my || !mz || !E) return fail(c, HARD_ERR_ARG, "hard_set_state: null pointer");
   int rc = ensure_ready(c);
   if (rc) return rc;
@@ -597,6 +618,7 @@ int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const doubl
 }
 
 int hard_get_state(hard_ctx* c, double* rho, double* mx, double* my, double* mz, double* E) {
+  DeviceGuard dg__(c);
   if (!c || !rho || !mx || !my || !mz || !E) return fail(c, HARD_ERR_ARG, "hard_get_state: null pointer");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
   double* dst[5] = { rho, mx, my, mz, E };
@@ -608,16 +630,19 @@ int hard_get_state(hard_ctx* c, double* rho, double* mx, double* my, double* mz,
 }
 
 int hard_step(hard_ctx* c, double cfl, int nsteps) {
+  DeviceGuard dg__(c);
   if (!c || !(cfl > 0.0) || nsteps < 0) return fail(c, HARD_ERR_ARG, "hard_step: cfl > 0 and nsteps >= 0 required");
   return do_steps(c, cfl, 0.0, nsteps);
 }
 
 int hard_step_dt(hard_ctx* c, double dt, int nsteps) {
+  DeviceGuard dg__(c);
   if (!c || !(dt > 0.0) || nsteps < 0) return fail(c, HARD_ERR_ARG, "hard_step_dt: dt > 0 and nsteps >= 0 required");
   return do_steps(c, 1.0, dt, nsteps);
 }
 
 int hard_max_dt(hard_ctx* c, double* dt_out) {
+  DeviceGuard dg__(c);
   if (!c || !dt_out) return fail(c, HARD_ERR_ARG, "hard_max_dt: null");
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
   DevScalars h;
@@ -629,6 +654,7 @@ int hard_max_dt(hard_ctx* c, double* dt_out) {
 }
 
 int hard_get_time(hard_ctx* c, double* t, long long* steps_done) {
+  DeviceGuard dg__(c);
   if (!c) return HARD_ERR_ARG;
   if (!c->have_state) return fail(c, HARD_ERR_NOSTATE, "no state");
   DevScalars h;
@@ -639,6 +665,7 @@ int hard_get_time(hard_ctx* c, double* t, long long* steps_done) {
 }
 
 int hard_stage_time(hard_ctx* c, int reset, double* ms, long long* launches) {
+  DeviceGuard dg__(c);
   if (!c) return HARD_ERR_ARG;
   CK(cudaStreamSynchronize(c->stream));
   double tot = 0.0;
