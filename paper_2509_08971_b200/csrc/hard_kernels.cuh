@@ -410,17 +410,34 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
     mbar_expect_tx(bar, C::BOX_BYTES);
     tma_load_4d(smem_u32(ring + slot * SLOT), &tmap, bar, cx, cy, g.off[2] + z, 0);
   };
-  auto wait_convert = [&](int z) {                     // all threads: wait, conserved -> primitive in place (a2)
+  auto convert_cell = [&](double* sl, int c) {
+    double U[5], W[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) U[v] = sl[v * VS + c];
+    cons_to_prim(U, gm1, W);
+#pragma unroll
+    for (int v = 1; v < 5; ++v) sl[v * VS + c] = W[v];
+  };
+  // all threads: wait for the plane, conserved -> primitive in place (a2).  Each thread converts first the cell
+  // of ITS OWN column (the only cell of the new plane that the next z reconstruction reads, and only this
+  // thread reads it), then a share of the halo ring, which nobody reads before the plane becomes the x/y
+  // plane several barriers later: no block-wide barrier is needed after the conversion when z is active.
+  auto wait_convert = [&](int z) {
     const int q = z - zb, slot = q % NS;
     mbar_wait(smem_u32(&bars[slot]), (uint32_t)((q / NS) & 1));
     double* sl = ring + slot * SLOT;
-    for (int c = tid; c < VS; c += C::NT) {
-      double U[5], W[5];
-#pragma unroll
-      for (int v = 0; v < 5; ++v) U[v] = sl[v * VS + c];
-      cons_to_prim(U, gm1, W);
-#pragma unroll
-      for (int v = 1; v < 5; ++v) sl[v * VS + c] = W[v];
+    convert_cell(sl, (ty + G) * BX + (tx - 1 + G));
+    constexpr int NTB = 2 * G * BX, NCOL = BX - 16, NREM = NTB + NCOL * TY;
+    for (int r = tid; r < NREM; r += C::NT) {
+      int row, col;
+      if (r < NTB) {
+        row = r / BX; col = r - row * BX;
+        row = row < G ? row : row + TY;
+      } else {
+        const int qq = r - NTB, rm = qq / NCOL, cc = qq - rm * NCOL;
+        row = G + rm; col = cc < G - 1 ? cc : cc + 16;
+      }
+      convert_cell(sl, row * BX + col);
     }
   };
 
@@ -548,7 +565,8 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
       }
     }
     if (more) wait_convert(znext);
-    __syncthreads();                                                             // barrier 3
+    // z inactive: the plane just converted is the next iteration's x/y plane, read by other threads at once
+    if (!az) __syncthreads();                                                    // barrier 3 (2-D / 1-D / x,y passes)
   }
   if (a.mode == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
 }
