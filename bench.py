@@ -33,8 +33,8 @@ ALG_BYTES_PER_CELL_STAGE = 100.0     # stage 1 = 40 R + 40 W, stage 2
 ALG_FLOP_PER_CELL_STAGE = {"A": 2600.0, "B": 1080.0}
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-1 launch at 896^3 from the committed ncu capture
-# (profiles/stage_A_r1_v4_ncu.txt, stage_B_r1_v4_ncu.txt); algorithmic bytes of that launch: 80 B x 896^3 = 57.5e9
-NCU_TRAFFIC_STAGE1_C4 = {"A": 38.247149e9 + 29.059888e9, "B": 34.260449e9 + 28.952542e9}
+# (profiles/stage_A_r1_v5_ncu.txt, stage_B_r1_v5_ncu.txt); algorithmic bytes of that launch: 80 B x 896^3 = 57.5e9
+NCU_TRAFFIC_STAGE1_C4 = {"A": 37.268129e9 + 28.982001e9, "B": 34.111760e9 + 28.935036e9}
 
 WORKLOADS = {"c4": (896, 10), "c3": (512, 20), "c2s": (256, 10)}
 
@@ -251,7 +251,7 @@ def run_cuda(args):
     roofline = {"bound": "alu", "kernel": "stage_kernel<%s>" % args.scheme, "achieved": alg_tflops, "peak": fp64_peak,
                 "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None,
                 "traffic": NCU_TRAFFIC_STAGE1_C4[args.scheme] if (args.workload == "c4" and variant == hard.VARIANT_FUSED) else None,
-                "traffic_note": "ncu dram bytes of one stage-1 launch (algorithmic: 80 B/cell = 57.5e9); profiles/stage_*_r1_v4_ncu.txt",
+                "traffic_note": "ncu dram bytes of one stage-1 launch (algorithmic: 80 B/cell = 57.5e9); profiles/stage_*_r1_v5_ncu.txt",
                 "peak_source": "measured live: hard_probe_fp64_peak (DFMA chains, all SMs)",
                 "avg_launch_ms": per_launch_ms, "launches_timed": stage_launches,
                 "alg_flop_per_cell_stage": ALG_FLOP_PER_CELL_STAGE[args.scheme]}
