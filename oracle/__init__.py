@@ -61,6 +61,7 @@ def lib():
         L.oracle_get_time.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
         L.oracle_fallback_count.restype = ctypes.c_longlong
         L.oracle_fallback_count.argtypes = [vp]
+        L.oracle_rhs.argtypes = [vp, dp]
         L.oracle_sum3sym.restype = ctypes.c_double
         L.oracle_sum3sym.argtypes = [ctypes.c_double] * 3
         L.oracle_wenoz.restype = ctypes.c_double
@@ -164,6 +165,12 @@ class Oracle:
         n = ctypes.c_longlong()
         self._chk(self.L.oracle_get_time(self.h, ctypes.byref(t), ctypes.byref(n)), "get_time")
         return t.value, n.value
+
+    def rhs(self, nf=5):
+        """L(U) of the current state (eq.15): list of nf arrays of shape (nz, ny, nx)."""
+        out = np.empty((nf,) + self.shape, dtype=np.float64)
+        self._chk(self.L.oracle_rhs(self.h, _dp(out)), "rhs")
+        return [out[f] for f in range(nf)]
 
     def fallbacks(self):
         return int(self.L.oracle_fallback_count(self.h))

@@ -23,15 +23,19 @@
 //   radiation energy density advected with the fluid, Rusanov    P:93 eq.2 (4th row), eq.14 LHS,
 //   (local Lax-Friedrichs) flux                                   P:151            (NEXT-1; G19)
 //   radiative heating q = c kappa rho (E_rad - a T^4), operator   P:66, eq.4,6
-//   split after the advection step, backward Euler                                 (NEXT-3; G20)
+//   split after the advection step, backward Euler, root by bisection             (NEXT-3; G20)
 // Every place where the paper is silent is a DESIGN.md reading (G1..G13) and is marked below.
 //
 // Pins (tests/test_oracle_*.py, all -m "not gpu"): exact Sod / LeBlanc Riemann solutions and L1
 // convergence, the paper's printed Sod bound, Sedov-Taylor shock radius, acoustic-wave
 // order, conservation to 1e-13, exact uniform-state preservation, bit-for-bit mirror
 // and axis-permutation symmetry, 1-D == replicated 3-D pencil, polynomial exactness of the WENO
-// candidate stencils, flux consistency F*(W,W) = F(W), stationary contact under HLLC, and a
-// hand-unrolled brute-force step on a 4x4x4 periodic grid.  No function here is "parity unpinned".
+// candidate stencils, flux consistency F*(W,W) = F(W), stationary contact under HLLC, a whole-array
+// restatement of a full step, and (tests/test_oracle_pins_r2.py, each failing under the matching mutation
+// of this file): wenoz against WENO5-Z rebuilt from its integral definition with numpy.polynomial;
+// outflow ghosts against the scalar upwind scheme that uniform-(u,p) flow reduces to; the G4 fallback
+// against textbook HLL fluxes of cell averages read off L(U) by telescoping.  No function here is
+// "parity unpinned".
 
 #include <algorithm>
 #include <cmath>
@@ -333,9 +337,11 @@ void rhs(Ctx* c, const std::vector<double> V[6], std::vector<double> Lout[6]) {
 // NEXT-3 (G20): the pointwise source update of the paper's operator split ("advection, diffusion, source
 // updates") restricted to the heating rate q = c kappa rho (E_rad - a T^4) (eq.6; force and
 // diffusion out of scope): d_t e = q, d_t E_rad = -q (eq.4), T = e / (rho c_v) (ideal gas).  Backward
-// Euler over dt conserves e + E_rad exactly: solve g(x) = x - e - dt c kappa rho (E_tot - x - a (x/(rho c_v))^4) = 0
-// for the new internal energy density x by Newton's method, safeguarded by the bracket [0, E_tot] on which
-// g is increasing and changes sign.
+// Euler over dt conserves e + E_rad exactly: the new internal energy density x is the root of
+//   g(x) = x - e - dt c kappa rho (E_tot - x - a (x/(rho c_v))^4)
+// on [0, E_tot], where g is increasing with g(0) <= 0 <= g(E_tot).  The oracle finds it the plainest way:
+// bisection until the bracket is two adjacent doubles (no Newton step, no tolerance), then the end with the
+// smaller |g|.  How the CUDA path iterates is its own business; parity compares the root.
 void apply_source(Ctx* c, double dt) {
   for (int k = 0; k < c->n[2]; ++k)
     for (int j = 0; j < c->n[1]; ++j)
@@ -347,17 +353,17 @@ void apply_source(Ctx* c, double dt) {
         double Etot = e + Er;
         double beta = dt * c->src_c * c->src_kappa * rho;
         double rcv = rho * c->src_cv;
-        double lo = 0.0, hi = Etot, x = e < 0.0 ? 0.0 : (e > Etot ? Etot : e);
-        for (int it = 0; it < 200; ++it) {
-          double T = x / rcv, T2 = T * T, T4 = T2 * T2;
-          double gx = (x - e) - beta * ((Etot - x) - c->src_a * T4);
-          if (gx > 0.0) hi = x; else lo = x;
-          double dg = 1.0 + beta * (1.0 + 4.0 * c->src_a * T2 * T / rcv);
-          double xn = x - gx / dg;
-          if (std::fabs(xn - x) <= 1e-15 * std::fabs(xn)) { x = xn; break; }   // converged (also onto a bracket end)
-          if (!(xn >= lo && xn <= hi)) xn = 0.5 * (lo + hi);           // Newton left the bracket: bisect
-          x = xn;
+        auto g = [&](double x) {
+          double T = x / rcv, T2 = T * T;
+          return (x - e) - beta * ((Etot - x) - c->src_a * (T2 * T2));
+        };
+        double lo = 0.0, hi = Etot;
+        for (int it = 0; it < 4000; ++it) {                      // 1075 halvings reach any double from [0, hi]
+          double mid = lo + 0.5 * (hi - lo);
+          if (!(mid > lo && mid < hi)) break;                    // lo and hi are adjacent doubles
+          if (g(mid) > 0.0) hi = mid; else lo = mid;
         }
+        double x = (std::fabs(g(lo)) <= std::fabs(g(hi))) ? lo : hi;
         c->U[4][p] = x + ke;
         c->U[5][p] = Etot - x;
       }
@@ -543,6 +549,19 @@ int oracle_get_time(void* h, double* t, long long* steps_done) {
 }
 
 long long oracle_fallback_count(void* h) { return h ? ((Ctx*)h)->fallbacks : -1; }
+
+// L(U) of the current state (eq.15), ghosts filled first; out holds nf arrays of nx*ny*nz doubles,
+// field-major.  Observability for the pins (tests read single face fluxes off it by telescoping).
+int oracle_rhs(void* h, double* out) {
+  Ctx* c = (Ctx*)h;
+  if (!c || !out) return ORC_ERR_ARG;
+  if (!c->have_state) return ORC_ERR_NOSTATE;
+  std::vector<double> L[6];
+  fill_ghosts(c, c->U);
+  rhs(c, c->U, L);
+  for (int f = 0; f < c->nf; ++f) std::copy(L[f].begin(), L[f].end(), out + (size_t)f * c->ncell());
+  return ORC_OK;
+}
 
 // Building blocks exposed so that tests can pin them one by one.
 double oracle_sum3sym(double a, double b, double c) { return sum3sym(a, b, c); }

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
+import _weno_def as wd
 from paper_2509_08971_b200 import workloads as wl
 
 SCHEMES = [0, 1]
@@ -145,14 +146,9 @@ def _np_step(st, g, sp, dt, scheme):
         p = (g - 1) * (U[4] - 0.5 * (U[1] * vel[0] + U[2] * vel[1] + U[3] * vel[2]))
         return [rho, vel[0], vel[1], vel[2], p]
 
-    def wz(a, b, c, d, e):
-        b0 = 13 / 12 * (a - 2 * b + c) ** 2 + 0.25 * (a - 4 * b + 3 * c) ** 2
-        b1 = 13 / 12 * (b - 2 * c + d) ** 2 + 0.25 * (b - d) ** 2
-        b2 = 13 / 12 * (c - 2 * d + e) ** 2 + 0.25 * (3 * c - 4 * d + e) ** 2
-        tau = np.abs(b0 - b2)
-        al = [0.1 * (1 + tau / (b0 + 1e-40)), 0.6 * (1 + tau / (b1 + 1e-40)), 0.3 * (1 + tau / (b2 + 1e-40))]
-        q = [(2 * a - 7 * b + 11 * c) / 6, (-b + 5 * c + 2 * d) / 6, (2 * c + 5 * d - e) / 6]
-        return (al[0] * q[0] + al[1] * q[1] + al[2] * q[2]) / (al[0] + al[1] + al[2])
+    # WENO5-Z from its integral definition (tests/_weno_def.py: parabolas, smoothness integrals and ideal
+    # weights derived with numpy.polynomial, pinned against the oracle in tests/test_oracle_pins_r2.py)
+    wz = wd.wenoz
 
     def L(U):
         W = prim(U)
