@@ -17,28 +17,29 @@ template <int S> struct SchemeTraits;
 template <> struct SchemeTraits<SCHEME_A> { static constexpr int G = 3, R = 2; };
 template <> struct SchemeTraits<SCHEME_B> { static constexpr int G = 2, R = 1; };
 
-// 1/x for normal, finite x: MUFU.RCP64H seed (about 20 good bits) + two Newton steps (4 DFMA), error
+// min / max of two finite doubles without the NaN bookkeeping of fmin / fmax (one DSETP + two selects
+// instead of DSETP.MIN + select + NaN fix-up + moves); callers pass finite values by construction.
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+
+// 1/x for normal, finite x: MUFU.RCP64H seed y (it reads only the upper 32 bits of x: relative error
+// e = 1 - x y below 2^-19) refined with the third-order step y (1 + e + e^2): 3 DFMA, remainder e^3 < 2^-57,
 // about 1 ulp; no special-case handling (the IEEE division sequence costs about 10 fp64-pipe
 // instructions).  Callers pass quantities that are normal by construction.
 __device__ __forceinline__ double fast_rcp(double x) {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-x, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-x, y, 1.0);
-  return fma(y, e, y);
+  const double e = fma(-x, y, 1.0);
+  return fma(y, fma(e, e, e), y);
 }
 
-// 1/sqrt(x) for normal, finite x > 0: MUFU.RSQ64H seed + two Newton steps (7 fp64-pipe instructions,
-// about 1 ulp), no special-case handling.
+// 1/sqrt(x) for normal, finite x > 0: MUFU.RSQ64H seed y, e = 1 - x y^2 (below 2^-18), third-order step
+// y (1 + e/2 + 3 e^2/8): 5 fp64-pipe instructions, remainder 5/16 e^3 < 2^-55, about 1 ulp.
 __device__ __forceinline__ double fast_rsqrt(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double h = 0.5 * x;
-  double e = fma(-h, y * y, 0.5);
-  y = fma(y, e, y);
-  e = fma(-h, y * y, 0.5);
-  return fma(y, e, y);
+  const double e = fma(-x, y * y, 1.0);
+  return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
 // a2 (eq.2): (rho, mx, my, mz, E) -> (rho, u, v, w, p).
@@ -58,12 +59,13 @@ __device__ __forceinline__ void cons_to_prim(const double U[5], double gm1, doub
 // arranged for the fp64 pipe:
 //  * everything in terms of the four differences d1..d4 (candidates minus c are 2-term forms);
 //  * beta scaled by 12/13 (beta' = s^2 + 3/13 t^2, eps' = 12/13 eps): tau/(beta+eps) is unchanged;
-//  * weights d_k (1 + tau/B_k) multiplied through by B0 B1 B2: d_k (B_k + tau) prod_{j!=k} B_j, which
-//    needs no division; ONE reciprocal 1/(sp*sm) normalises both sides.
-//    Range: B in [9e-41, ~1e17] for admissible data of the configs, so products of three B's and the
-//    square of their sum stay within [1e-241, 1e110]: no overflow / underflow in fp64.
-__device__ __forceinline__ void wenoz_pair(double a, double b, double c, double d, double e, double& plus,
-                                           double& minus) {
+//  * weights d_k (1 + tau/B_k) multiplied through by 10 B0 B1 B2: X_k = (B_k + tau) prod_{j!=k} B_j with the
+//    integer multipliers (1, 6, 3), which needs no division; one reciprocal per face normalises.
+//    Range: the X are cubic in B, so data up to about 1e51 in magnitude neither overflow nor (B >= 9e-41)
+//    underflow.
+//  * returned: the increments 6 (plus - c) and 6 (minus - c); the caller adds c back with the factor 1/6 — or
+//    with the factor 0 where the positivity fallback (G4) applies, which costs nothing.
+__device__ __forceinline__ void wenoz_incr(double a, double b, double c, double d, double e, double& wp, double& wm) {
   const double eps = (12.0 / 13.0) * 1e-40, k3 = 3.0 / 13.0;
   const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
   const double s0 = d2 - d1, s1 = d3 - d2, s2 = d4 - d3;
@@ -72,34 +74,29 @@ __device__ __forceinline__ void wenoz_pair(double a, double b, double c, double 
   const double B1 = fma(s1, s1, fma(k3 * t1, t1, eps));
   const double B2 = fma(s2, s2, fma(k3 * t2, t2, eps));
   const double tau = fabs(B0 - B2);
-  const double P12 = B1 * B2, P02 = B0 * B2, P01 = B0 * B1;
-  const double T0 = B0 + tau, T1 = B1 + tau, T2 = B2 + tau;
-  const double a0 = (0.1 * T0) * P12, a1 = (0.6 * T1) * P02;                // plus weights (unnormalised)
-  const double m0 = (0.1 * T2) * P01;                                       // minus weights; m1 = a1
-  const double a2 = 3.0 * m0, m2 = 3.0 * a0;                                // 0.3 T2 P01 and 0.3 T0 P12
-  const double sp = (a0 + a1) + a2, sm = (m0 + a1) + m2;
+  const double X0 = (B0 + tau) * (B1 * B2), X1 = (B1 + tau) * (B0 * B2), X2 = (B2 + tau) * (B0 * B1);
+  const double Y = 6.0 * X1, X0t = 3.0 * X0, X2t = 3.0 * X2;
+  const double sp = (X0 + Y) + X2t, sm = (X2 + Y) + X0t;             // 10 x (sum of the unnormalised weights)
   // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
   const double q0 = fma(5.0, d2, -2.0 * d1), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);
   const double p0 = fma(-5.0, d3, 2.0 * d4), p1 = -fma(2.0, d2, d3), p2 = fma(-4.0, d2, d1);
-  const double np = fma(a2, q2, fma(a1, q1, a0 * q0));
-  const double nm = fma(m2, p2, fma(a1, p1, m0 * p0));
-  const double inv6 = (1.0 / 6.0) * fast_rcp(sp * sm);
-  plus = fma(np, inv6 * sm, c);
-  minus = fma(nm, inv6 * sp, c);
+  const double np = fma(X2t, q2, fma(Y, q1, X0 * q0));
+  const double nm = fma(X0t, p2, fma(Y, p1, X2 * p0));
+  wp = np * fast_rcp(sp);
+  wm = nm * fast_rcp(sm);
 }
 
-// a3, scheme B: MUSCL with the minmod limiter.  Branch-free: the slope is min(|x|,|y|) with the sign
-// of x when x and y have the same sign (test on the sign bits, integer pipe) and 0 otherwise —
-// the same value as the sign-test definition for all finite inputs (x or y = 0 gives 0).
+// a3, scheme B: MUSCL with the minmod limiter.  Branch-free: the slope is the argument of smaller
+// magnitude when x and y have the same sign (test on the sign bits, integer pipe) and 0 otherwise —
+// the same value as the sign-test definition for all finite inputs (x or y = 0 gives 0).  The zero
+// case is folded into the factor 1/2 (its high word is selected, the low word is zero either way).
 __device__ __forceinline__ void minmod_pair(double b, double c, double d, double& plus, double& minus) {
   const double x = c - b, y = d - c;
-  const double m = fmin(fabs(x), fabs(y));
-  const int hx = __double2hiint(x), hy = __double2hiint(y);
-  const int hm = ((hx ^ hy) < 0) ? 0 : (__double2hiint(m) | (hx & 0x80000000));
-  const int lm = ((hx ^ hy) < 0) ? 0 : __double2loint(m);
-  const double s = __hiloint2double(hm, lm);
-  plus = fma(0.5, s, c);
-  minus = fma(-0.5, s, c);
+  const double s = fabs(x) < fabs(y) ? x : y;
+  const int hh = ((__double2hiint(x) ^ __double2hiint(y)) < 0) ? 0 : 0x3fe00000;       // 0.0 or 0.5
+  const double h = __hiloint2double(hh, 0);
+  plus = fma(h, s, c);
+  minus = fma(-h, s, c);
 }
 
 // a4 (G2 Davis bounds; G5 inclusive tie-breaks).  WL/WR = (rho, un, ut1, ut2, p) already
@@ -112,73 +109,70 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
   const double gpL = gamma * WL[4], gpR = gamma * WR[4];
   const double cL = gpL * fast_rsqrt(gpL * WL[0]);
   const double cR = gpR * fast_rsqrt(gpR * WR[0]);
-  const double SL = fmin(WL[1] - cL, WR[1] - cR);
-  const double SR = fmax(WL[1] + cL, WR[1] + cR);
-  alpha = fmax(SR, -SL);                                 // = max(|u_n| + c_s) over the two sides (Rusanov, NEXT-1)
+  const double SL = dmin(WL[1] - cL, WR[1] - cR);
+  const double SR = dmax(WL[1] + cL, WR[1] + cR);
+  alpha = dmax(SR, -SL);                                 // = max(|u_n| + c_s) over the two sides (Rusanov, NEXT-1)
   if (S == SCHEME_A) {                                   // HLL needs both sides' U and F
-    const double EL = WL[4] * inv_gm1 + 0.5 * WL[0] * (WL[1] * WL[1] + (WL[2] * WL[2] + WL[3] * WL[3]));
-    const double ER = WR[4] * inv_gm1 + 0.5 * WR[0] * (WR[1] * WR[1] + (WR[2] * WR[2] + WR[3] * WR[3]));
+    const double EL = fma(0.5 * WL[0], fma(WL[1], WL[1], fma(WL[2], WL[2], WL[3] * WL[3])), WL[4] * inv_gm1);
+    const double ER = fma(0.5 * WR[0], fma(WR[1], WR[1], fma(WR[2], WR[2], WR[3] * WR[3])), WR[4] * inv_gm1);
     const double UL[5] = { WL[0], WL[0] * WL[1], WL[0] * WL[2], WL[0] * WL[3], EL };
     const double UR[5] = { WR[0], WR[0] * WR[1], WR[0] * WR[2], WR[0] * WR[3], ER };
-    const double FL[5] = { UL[1], UL[1] * WL[1] + WL[4], UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
-    const double FR[5] = { UR[1], UR[1] * WR[1] + WR[4], UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
-    if (SL >= 0.0) {
+    const double FL[5] = { UL[1], fma(UL[1], WL[1], WL[4]), UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
+    const double FR[5] = { UR[1], fma(UR[1], WR[1], WR[4]), UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
+    // Branch-free: with SL- = min(SL, 0), SR+ = max(SR, 0) the HLL formula returns F_L when SL >= 0 and F_R when
+    // SR <= 0 (G5's inclusive tie-breaks, to rounding); c > 0 keeps SR+ - SL- > 0.
+    const double SLm = dmin(SL, 0.0), SRp = dmax(SR, 0.0);
+    const double inv = fast_rcp(SRp - SLm);
+    const double wl = SRp * inv, wr = SLm * inv, ws = wl * SLm;
 #pragma unroll
-      for (int m = 0; m < 5; ++m) F[m] = FL[m];
-      return;
-    }
-    if (SR <= 0.0) {
-#pragma unroll
-      for (int m = 0; m < 5; ++m) F[m] = FR[m];
-      return;
-    }
-    const double inv = fast_rcp(SR - SL);
-    const double ss = SL * SR;
-#pragma unroll
-    for (int m = 0; m < 5; ++m) F[m] = ((SR * FL[m] - SL * FR[m]) + ss * (UR[m] - UL[m])) * inv;
+    for (int m = 0; m < 5; ++m) F[m] = fma(ws, UR[m] - UL[m], fma(-wr, FR[m], wl * FL[m]));
   } else {
     // HLLC, averaged-pressure form (G5).  Only the upwind side's U and F enter the result: side L if
     // SL >= 0 or (SR > 0 and S* > 0), else side R; the supersonic cases return that side's F.
     const double A = WL[0] * (SL - WL[1]);
     const double B = WR[0] * (SR - WR[1]);
-    const double Ss = ((WR[4] - WL[4]) + (A * WL[1] - B * WR[1])) * fast_rcp(A - B);
-    const double pbar = 0.5 * ((WL[4] + WR[4]) + (A * (Ss - WL[1]) + B * (Ss - WR[1])));
-    const bool supL = SL >= 0.0, supR = !supL && SR <= 0.0;
-    const bool left = supL || (!supR && Ss > 0.0);
+    const double Ss = ((WR[4] - WL[4]) + fma(A, WL[1], -B * WR[1])) * fast_rcp(A - B);
+    const double pbar = 0.5 * ((WL[4] + WR[4]) + fma(A, Ss - WL[1], B * (Ss - WR[1])));
+    // S* lies strictly between SL and SR, so SL >= 0 implies S* > 0 and SR <= 0 implies S* < 0: "left" covers the
+    // supersonic cases too.  F* = F_K + S_K (U*_K - U_K) with U*_K - U_K = (S* U_K - F_K + pbar D*) / (S_K - S*)
+    // — the same flux as the averaged-pressure quotient, regrouped — and S_K clamped to zero on the supersonic
+    // side returns F_K itself: no branch, no select on the result.
+    const bool left = Ss > 0.0;
     double W[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) W[m] = left ? WL[m] : WR[m];
     const double SK = left ? SL : SR;
-    const double E = W[4] * inv_gm1 + 0.5 * W[0] * (W[1] * W[1] + (W[2] * W[2] + W[3] * W[3]));
+    const bool sub = left ? (SK < 0.0) : (SK > 0.0);
+    const double SKc = sub ? SK : 0.0;
+    const double E = fma(0.5 * W[0], fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3])), W[4] * inv_gm1);
     const double UK[5] = { W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E };
-    const double FK[5] = { UK[1], UK[1] * W[1] + W[4], UK[1] * W[2], UK[1] * W[3], (E + W[4]) * W[1] };
-    // Branch-free tail: S* = 0 needs no special case here (the formula gives (0, pbar, 0, 0, 0) exactly:
-    // every term carries the factor S* except SK pbar / SK), and the supersonic cases select F_K.
-    const bool sup = supL || supR;
-    const double inv = fast_rcp(SK - Ss);
-    const double sp = SK * pbar;
+    const double FK[5] = { UK[1], fma(UK[1], W[1], W[4]), UK[1] * W[2], UK[1] * W[3], (E + W[4]) * W[1] };
+    const double g = SKc * fast_rcp(SK - Ss);
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
-      double t = Ss * (SK * UK[m] - FK[m]);
-      if (m == 1) t += sp;
-      if (m == 4) t = fma(sp, Ss, t);
-      F[m] = sup ? FK[m] : t * inv;
+      double t = fma(Ss, UK[m], -FK[m]);
+      if (m == 1) t += pbar;
+      if (m == 4) t = fma(pbar, Ss, t);
+      F[m] = fma(g, t, FK[m]);
     }
   }
 }
 
 // a7 building block for the fused epilogue: local max wavespeed of one conserved state; returns a
-// negative value if the state is not admissible (non-finite, rho <= 0 or p <= 0).
+// negative value if the state is not admissible (non-finite, rho <= 0 or p <= 0).  The next step's dt
+// inherits the state's rounding differences anyway (G9: compared at 1e-9), so this uses the fast
+// reciprocal / rsqrt forms; the standalone cfl_kernel keeps the correctly rounded definition.
 __device__ __forceinline__ double cell_lambda(const double U[5], double gamma, double gm1, const double inv_d[3],
                                               const bool act[3]) {
   double W[5];
   cons_to_prim(U, gm1, W);
   if (!(W[0] > 0.0 && W[4] > 0.0) || !(W[4] < 1.0e300)) return -1.0;
-  const double c = sqrt(gamma * W[4] / W[0]);
+  const double gp = gamma * W[4];
+  const double c = gp * fast_rsqrt(gp * W[0]);
   double lam = 0.0;
 #pragma unroll
   for (int a = 0; a < 3; ++a)
-    if (act[a]) lam = fmax(lam, (fabs(W[1 + a]) + c) * inv_d[a]);
+    if (act[a]) lam = dmax(lam, (fabs(W[1 + a]) + c) * inv_d[a]);
   return lam;
 }
 

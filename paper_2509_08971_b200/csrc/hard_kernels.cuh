@@ -330,24 +330,34 @@ struct StageCfg {
 };
 
 // Both face values of all five primitives of one cell along one direction; o[s] = ring offset of
-// field 0 at stencil position s - R.  Scheme A applies the positivity fallback (G4).
+// field 0 at stencil position s - R.  Scheme A applies the positivity fallback (G4): if a reconstructed rho
+// or p is <= 0, all variables of the cell become piecewise constant — done by adding the WENO increments
+// with the factor 0 instead of 1/6, so the fallback costs four extra DFMA and no branch.  "<= 0" is taken on
+// the high words (sign set, or zero): exact for every value but a positive denormal, which no admissible
+// state reconstructs.
 template <int S, int NF>
 __device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double* pl, double* mi) {
   constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S, NF>::VS;
-#pragma unroll
-  for (int v = 0; v < NF; ++v) {
-    if (S == SCHEME_A) {
-      wenoz_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], ring[o[3] + v * VS],
-                 ring[o[4] + v * VS], pl[v], mi[v]);
-    } else {
-      minmod_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], pl[v], mi[v]);
-    }
-  }
   if (S == SCHEME_A) {
-    if (pl[0] <= 0.0 || pl[4] <= 0.0 || mi[0] <= 0.0 || mi[4] <= 0.0) {
+    double c[NF], wp[NF], wm[NF];
+    constexpr int order[6] = { 0, 4, 1, 2, 3, 5 };       // rho and p first: they decide the fallback
+    int hmin = 0x7fffffff;
+    double f6 = 1.0 / 6.0;
 #pragma unroll
-      for (int v = 0; v < NF; ++v) pl[v] = mi[v] = ring[o[R] + v * VS];     // G19: E_rad follows
+    for (int q = 0; q < NF; ++q) {
+      const int v = order[q];
+      c[v] = ring[o[2] + v * VS];
+      wenoz_incr(ring[o[0] + v * VS], ring[o[1] + v * VS], c[v], ring[o[3] + v * VS], ring[o[4] + v * VS], wp[v], wm[v]);
+      if (q < 2)
+        hmin = min(hmin, min(__double2hiint(fma(wp[v], 1.0 / 6.0, c[v])), __double2hiint(fma(wm[v], 1.0 / 6.0, c[v]))));
+      if (q == 1) f6 = hmin <= 0 ? 0.0 : 1.0 / 6.0;
     }
+#pragma unroll
+    for (int v = 0; v < NF; ++v) { pl[v] = fma(wp[v], f6, c[v]); mi[v] = fma(wm[v], f6, c[v]); }
+  } else {
+#pragma unroll
+    for (int v = 0; v < NF; ++v)
+      minmod_pair(ring[o[0] + v * VS], ring[o[1] + v * VS], ring[o[2] + v * VS], pl[v], mi[v]);
   }
 }
 
@@ -561,7 +571,7 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
       }
       if (a.mode == MODE_STAGE2 && !a.skip_cfl) {
         const double l = cell_lambda(out, gamma, gm1, g.inv_d, act3);
-        if (l < 0.0) bad = 1; else lam_loc = fmax(lam_loc, l);
+        if (l < 0.0) bad = 1; else lam_loc = dmax(lam_loc, l);
       }
     }
     if (more) wait_convert(znext);
