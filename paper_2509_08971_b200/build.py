@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libhard_b200.so")
 SOURCES = ["hard_api.cu", "hard_probe.cu"]
-DEPS = ["hard_api.cu", "hard_probe.cu", "hard_kernels.cuh", "hard_device.cuh", os.path.join("..", "..", "include", "hard.h")]
+DEPS = ["hard_api.cu", "hard_probe.cu", "hard_kernels.cuh", "hard_stage3d.cuh", "hard_device.cuh", os.path.join("..", "..", "include", "hard.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -196,7 +196,9 @@ int ensure_ready(hard_ctx* c) {
     rc = make_map(c, &c->tmU1, c->U1);
     if (rc) return rc;
 #define HARD_SET_SMEM(S, NF) \
-  CK(cudaFuncSetAttribute(stage_kernel<S, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM));
+  CK(cudaFuncSetAttribute(stage_kernel<S, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM)); \
+  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM)); \
+  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM));
     HARD_SET_SMEM(SCHEME_A, 5) HARD_SET_SMEM(SCHEME_B, 5) HARD_SET_SMEM(SCHEME_A, 6) HARD_SET_SMEM(SCHEME_B, 6)
 #undef HARD_SET_SMEM
     c->Lz = choose_Lz(c);
@@ -260,8 +262,15 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
   dim3 grid((g.n[0] + 13) / 14, (g.n[1] + 15) / 16, (g.n[2] + a.Lz - 1) / a.Lz);
   int rc = prof_begin(c);
   if (rc) return rc;
+  // 3-D meshes with all fluxes in one launch take the specialised kernel (hard_stage3d.cuh)
+  static const bool generic_only = getenv("HARD_GENERIC_STAGE") != nullptr;
+  const bool spec3d = !generic_only && g.act[0] && g.act[1] && g.act[2] && dirmask == 7 && (mode == MODE_STAGE1 || mode == MODE_STAGE2);
 #define HARD_LAUNCH(S, NF) \
-  stage_kernel<S, NF><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a)
+  do { \
+    if (spec3d && mode == MODE_STAGE1) stage3d_kernel<S, NF, MODE_STAGE1><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
+    else if (spec3d) stage3d_kernel<S, NF, MODE_STAGE2><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
+    else stage_kernel<S, NF><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
+  } while (0)
   if (c->scheme == HARD_SCHEME_WENO5Z_HLL) { if (c->nf == 6) HARD_LAUNCH(SCHEME_A, 6); else HARD_LAUNCH(SCHEME_A, 5); }
   else                                     { if (c->nf == 6) HARD_LAUNCH(SCHEME_B, 6); else HARD_LAUNCH(SCHEME_B, 5); }
 #undef HARD_LAUNCH

@@ -581,4 +581,6 @@ stage_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict_
   if (a.mode == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
 }
 
+#include "hard_stage3d.cuh"
+
 }  // namespace hard

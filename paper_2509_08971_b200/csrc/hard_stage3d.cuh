@@ -1,0 +1,214 @@
+// hard_stage3d.cuh — the fused RK stage (a2..a7) specialised for the 3-D case: all three directions
+// active, all fluxes in one launch, the stage (1 or 2) a template parameter.  Same tiling, ring, thread
+// mapping and phase order as the generic stage_kernel (hard_kernels.cuh), which keeps serving 1-D / 2-D
+// meshes and the per-direction variant; what the specialisation buys is straight-line code between the
+// two barriers of a plane (ptxas interleaves the serial Riemann chains with the reconstruction of the
+// next phase), loop-carried z state that is updated in place (no register copies at the back edge), and no
+// per-phase activity tests.  Included by hard_kernels.cuh inside namespace hard.
+#pragma once
+
+template <int S, int NF, int MODE>
+__global__ void __launch_bounds__(256, (StageCfg<S, NF>::CTAS))
+stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict__ Usrc, const double* Uaux,
+               double* Uout, GridDesc g, DevScalars* sc, StageArgs a) {
+  using C = StageCfg<S, NF>;
+  constexpr int G = C::G, R = C::R, TX = C::TX, TY = C::TY, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS,
+                NYI = C::NYI;
+  constexpr bool LATE = (R >= 2);          // no spare ring slot: the next plane is requested after the z reconstruction
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double* ring = reinterpret_cast<double*>(smem_raw);
+  double* RMy = ring + NS * SLOT;      // y minus values, item-indexed [v][item]
+  double* Fy = RMy + NF * NYI;         // y face fluxes: item's upper face
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + NF * NYI);
+  double* red = reinterpret_cast<double*>(bars + NS);
+
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, k0 = blockIdx.z * a.Lz;
+  const int kend = min(g.n[2], k0 + a.Lz);
+  const int rows = min(TY, g.n[1] - j0), cols = min(TX, g.n[0] - i0);
+  const bool mine = tx >= 1 && tx <= cols && ty < rows;          // thread tx owns cell ix = tx - 1
+  // y items: cells (y_ix, y_c - 1), y_c = 0..TY+1; the last four threads repeat item NYI-1 (nothing stored)
+  const int yit = min(tid, NYI - 1), y_c = yit / TX, y_ix = yit - y_c * TX;
+  const bool ystore = tid < NYI;
+  const double gamma = g.gamma, gm1 = gamma - 1.0, inv_gm1 = 1.0 / gm1;
+  const double dt = step_dt(sc, a.cur, a.cfl, a.dt_fixed);
+  const double idx = g.inv_d[0], idy = g.inv_d[1], idz = g.inv_d[2];
+  const int zb = k0 - R - 1;                                     // first plane loaded; ring slot of plane z = (z - zb) % NS
+  const int cx = g.off[0] + i0 - G, cy = g.off[1] + j0 - G;      // cx = i0: even, so 16-byte aligned
+  const int cellz = (ty + G) * BX + (tx - 1 + G);                // own column (also the x item of this thread)
+  const int celly = (y_c - 1 + G) * BX + (y_ix + G);
+
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) mbar_init(smem_u32(&bars[s]), 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  auto issue = [&](int z) {                            // one thread
+    const int q = z - zb, slot = q % NS;
+    const uint32_t bar = smem_u32(&bars[slot]);
+    mbar_expect_tx(bar, C::BOX_BYTES);
+    tma_load_4d(smem_u32(ring + slot * SLOT), &tmap, bar, cx, cy, g.off[2] + z, 0);
+  };
+  auto convert_cell = [&](double* sl, int c) {
+    double U[5], W[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) U[v] = sl[v * VS + c];
+    cons_to_prim(U, gm1, W);
+#pragma unroll
+    for (int v = 1; v < 5; ++v) sl[v * VS + c] = W[v];
+  };
+  // wait for the plane, conserved -> primitive in place (a2): own column first (see stage_kernel), then a share of the halo
+  auto wait_convert = [&](int z) {
+    const int q = z - zb, slot = q % NS;
+    mbar_wait(smem_u32(&bars[slot]), (uint32_t)((q / NS) & 1));
+    double* sl = ring + slot * SLOT;
+    convert_cell(sl, cellz);
+    constexpr int NTB = 2 * G * BX, NCOL = BX - 16, NREM = NTB + NCOL * TY;
+    for (int r = tid; r < NREM; r += C::NT) {
+      int row, col;
+      if (r < NTB) {
+        row = r / BX; col = r - row * BX;
+        row = row < G ? row : row + TY;
+      } else {
+        const int qq = r - NTB, rm = qq / NCOL, cc = qq - rm * NCOL;
+        row = G + rm; col = cc < G - 1 ? cc : cc + 16;
+      }
+      convert_cell(sl, row * BX + col);
+    }
+  };
+
+  if (tid == 0)
+    for (int z = zb; z <= zb + 2 * R; ++z) issue(z);
+  for (int z = zb; z <= zb + 2 * R; ++z) wait_convert(z);
+  __syncthreads();
+
+  // loop-carried z state of the own column: plus value of the last reconstructed plane, and the flux through
+  // the last face already multiplied by 1/dz
+  double zplus[NF], Cz[NF];
+#pragma unroll
+  for (int v = 0; v < NF; ++v) { zplus[v] = (v == 0 || v == 4) ? 1.0 : 0.0; Cz[v] = 0.0; }
+  double lam_loc = 0.0;
+  int bad = 0;
+  const bool act3[3] = { true, true, true };
+
+  // z: reconstruct plane kk+1 (own column), flux through face kk+1/2 with the carried plus value.
+  // p = ring slot of plane kk.  Lz = -(F(kk+1/2) - F(kk-1/2)) / dz.
+  auto zphase = [&](int p, double* Lz) {
+    int o[2 * R + 1];
+#pragma unroll
+    for (int s = -R; s <= R; ++s) {
+      int sl = p + 1 + s;                               // in [1 - R, NS + R]
+      sl = sl < 0 ? sl + NS : (sl >= NS ? sl - NS : sl);
+      o[s + R] = sl * SLOT + cellz;
+    }
+    double pl[NF], mi[NF], F[NF];
+    recon_item<S, NF>(ring, o, pl, mi);
+    face_flux<S, 2, NF>(zplus, mi, gamma, inv_gm1, F);
+#pragma unroll
+    for (int v = 0; v < NF; ++v) {
+      const double Cn = __dmul_rn(F[v], idz);           // rounded product, never contracted: equal fluxes cancel
+      Lz[v] = Cz[v] - Cn;                               // exactly (a uniform state is preserved bit for bit)
+      Cz[v] = Cn;
+      zplus[v] = pl[v];
+    }
+  };
+
+  int p = R - 1;                                        // slot of plane kk = k0 - 2
+  // ---- two lead-in planes: z only
+  for (int kk = k0 - 2; kk < k0; ++kk) {
+    const int znext = kk + 2 + R;
+    if (!LATE && tid == 0) { fence_proxy_async(); issue(znext); }
+    double Lz[NF];
+    zphase(p, Lz);
+    __syncthreads();
+    if (LATE && tid == 0) { fence_proxy_async(); issue(znext); }
+    wait_convert(znext);
+    p = (p + 1 == NS) ? 0 : p + 1;
+  }
+
+  for (int kk = k0; kk < kend; ++kk) {
+    const int znext = kk + 2 + R;
+    const bool more = kk + 1 < kend;
+    if (!LATE && more && tid == 0) { fence_proxy_async(); issue(znext); }
+    const int slot_c = p * SLOT;                        // plane kk (x/y stencils)
+    double Lacc[NF];
+    zphase(p, Lacc);
+    // ---- y: reconstruct the 14 x 18 items of plane kk; minus values to shared memory
+    double plY[NF];
+    {
+      int o[2 * R + 1];
+#pragma unroll
+      for (int s = -R; s <= R; ++s) o[s + R] = slot_c + celly + s * BX;
+      double mi[NF];
+      recon_item<S, NF>(ring, o, plY, mi);
+      if (ystore) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) RMy[v * NYI + tid] = mi[v];
+      }
+    }
+    __syncthreads();                                                             // barrier 1
+    if (LATE && more && tid == 0) { fence_proxy_async(); issue(znext); }
+
+    // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
+    {
+      double pl[NF], mi[NF], mr[NF], F[NF];
+      int o[2 * R + 1];
+#pragma unroll
+      for (int s = -R; s <= R; ++s) o[s + R] = slot_c + cellz + s;
+      recon_item<S, NF>(ring, o, pl, mi);
+#pragma unroll
+      for (int v = 0; v < NF; ++v) mr[v] = __shfl_down_sync(0xffffffffu, mi[v], 1, 16);   // minus of cell tx
+      face_flux<S, 0, NF>(pl, mr, gamma, inv_gm1, F);                                        // face right of cell tx-1
+#pragma unroll
+      for (int v = 0; v < NF; ++v) {
+        const double Fl = __shfl_up_sync(0xffffffffu, F[v], 1, 16);                      // face left of cell tx-1
+        Lacc[v] = fma(Fl - F[v], idx, Lacc[v]);
+      }
+    }
+    // own-cell conserved values for the RK combination (consumed after barrier 2)
+    double uc[NF], ua[NF];
+    const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
+    if (mine) {
+#pragma unroll
+      for (int v = 0; v < NF; ++v) uc[v] = Usrc[v * g.fstride + pc];
+      if (MODE == MODE_STAGE2) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) ua[v] = Uaux[v * g.fstride + pc];
+      }
+    }
+    // ---- y fluxes: face above item (between item and item + TX); the top row's result is not used
+    {
+      double mr[NF], F[NF];
+      const int up = min(tid + TX, NYI - 1);
+#pragma unroll
+      for (int v = 0; v < NF; ++v) mr[v] = RMy[v * NYI + up];
+      face_flux<S, 1, NF>(plY, mr, gamma, inv_gm1, F);
+      if (ystore) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) Fy[v * NYI + tid] = F[v];
+      }
+    }
+    __syncthreads();                                                             // barrier 2
+
+    // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
+    if (mine) {
+      double out[NF];
+      const int yi = ty * TX + (tx - 1);               // item of cell (tx-1, ty-1): its upper face is our lower face
+#pragma unroll
+      for (int v = 0; v < NF; ++v) {
+        const double L = fma(Fy[v * NYI + yi] - Fy[v * NYI + yi + TX], idy, Lacc[v]);
+        if (MODE == MODE_STAGE1) out[v] = fma(dt, L, uc[v]);
+        else out[v] = 0.5 * ua[v] + 0.5 * fma(dt, L, uc[v]);
+        Uout[v * g.fstride + pc] = out[v];
+      }
+      if (MODE == MODE_STAGE2 && !a.skip_cfl) {
+        const double l = cell_lambda(out, gamma, gm1, g.inv_d, act3);
+        if (l < 0.0) bad = 1; else lam_loc = dmax(lam_loc, l);
+      }
+    }
+    if (more) wait_convert(znext);
+    p = (p + 1 == NS) ? 0 : p + 1;
+  }
+  if (MODE == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
+}
