@@ -7,6 +7,28 @@
 // per-phase activity tests.  Included by hard_kernels.cuh inside namespace hard.
 #pragma once
 
+#ifndef HARD_LDG_POS
+#define HARD_LDG_POS 0
+#endif
+__device__ __forceinline__ double ldg_pinned(const double* p) {
+  double v;
+  asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+
+#ifndef HARD_SPLIT_BAR
+#define HARD_SPLIT_BAR 1
+#endif
+#ifndef HARD_LATE_FULLBAR
+#define HARD_LATE_FULLBAR 1
+#endif
+// Split-phase CTA barrier on an mbarrier (8 arrivals: one elected lane per warp): arrive after producing,
+// wait just before consuming, with independent work in between, so that no warp idles for the slowest one.
+__device__ __forceinline__ void warp_arrive(uint32_t bar) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
 template <int S, int NF, int MODE>
 __global__ void __launch_bounds__(256, (StageCfg<S, NF>::CTAS))
 stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restrict__ Usrc, const double* Uaux,
@@ -38,8 +60,12 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   const int cellz = (ty + G) * BX + (tx - 1 + G);                // own column (also the x item of this thread)
   const int celly = (y_c - 1 + G) * BX + (y_ix + G);
 
+  // red[62], red[63] (unused by the final reduction) hold the two split-phase barriers of the plane loop
+  const uint32_t barY = smem_u32(&red[62]), barF = smem_u32(&red[63]);
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) mbar_init(smem_u32(&bars[s]), 1);
+    mbar_init(barY, 8);
+    mbar_init(barF, 8);
     fence_mbar_init();
   }
   __syncthreads();
@@ -127,6 +153,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     p = (p + 1 == NS) ? 0 : p + 1;
   }
 
+  uint32_t ph = 0;                                      // phase parity of the two split-phase barriers
   for (int kk = k0; kk < kend; ++kk) {
     const int znext = kk + 2 + R;
     const bool more = kk + 1 < kend;
@@ -147,9 +174,37 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         for (int v = 0; v < NF; ++v) RMy[v * NYI + tid] = mi[v];
       }
     }
+#if HARD_SPLIT_BAR
+    if (LATE && HARD_LATE_FULLBAR) {
+      __syncthreads();                                 // the oldest plane is free once every warp is past its z reconstruction
+      if (more && tid == 0) { fence_proxy_async(); issue(znext); }
+    } else {
+      warp_arrive(barY);                                                         // barrier 1, arrive: RMy written
+      if (LATE && more && tid == 0) {
+        mbar_wait(barY, ph);
+        fence_proxy_async();
+        issue(znext);
+      }
+    }
+#else
     __syncthreads();                                                             // barrier 1
     if (LATE && more && tid == 0) { fence_proxy_async(); issue(znext); }
+#endif
 
+    // own-cell conserved values for the RK combination (consumed after barrier 2), requested here so that the
+    // whole x phase covers their latency; volatile asm keeps ptxas from sinking them to the point of use.
+    double uc[NF], ua[NF];
+    const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
+#if HARD_LDG_POS == 0
+    if (mine) {
+#pragma unroll
+      for (int v = 0; v < NF; ++v) uc[v] = ldg_pinned(Usrc + v * g.fstride + pc);
+      if (MODE == MODE_STAGE2) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
+      }
+    }
+#endif
     // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
     {
       double pl[NF], mi[NF], mr[NF], F[NF];
@@ -166,18 +221,10 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         Lacc[v] = fma(Fl - F[v], idx, Lacc[v]);
       }
     }
-    // own-cell conserved values for the RK combination (consumed after barrier 2)
-    double uc[NF], ua[NF];
-    const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
-    if (mine) {
-#pragma unroll
-      for (int v = 0; v < NF; ++v) uc[v] = Usrc[v * g.fstride + pc];
-      if (MODE == MODE_STAGE2) {
-#pragma unroll
-        for (int v = 0; v < NF; ++v) ua[v] = Uaux[v * g.fstride + pc];
-      }
-    }
     // ---- y fluxes: face above item (between item and item + TX); the top row's result is not used
+#if HARD_SPLIT_BAR
+    if (!(LATE && HARD_LATE_FULLBAR)) mbar_wait(barY, ph);                       // barrier 1, wait: the x phase lay in between
+#endif
     {
       double mr[NF], F[NF];
       const int up = min(tid + TX, NYI - 1);
@@ -189,7 +236,14 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         for (int v = 0; v < NF; ++v) Fy[v * NYI + tid] = F[v];
       }
     }
+#if HARD_SPLIT_BAR
+    warp_arrive(barF);                                                           // barrier 2, arrive: Fy written
+    if (more) wait_convert(znext);                     // independent of Fy: covers the other warps' arrival
+    mbar_wait(barF, ph);                                                         // barrier 2, wait
+    ph ^= 1u;
+#else
     __syncthreads();                                                             // barrier 2
+#endif
 
     // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
     if (mine) {
@@ -207,7 +261,9 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         if (l < 0.0) bad = 1; else lam_loc = dmax(lam_loc, l);
       }
     }
+#if !HARD_SPLIT_BAR
     if (more) wait_convert(znext);
+#endif
     p = (p + 1 == NS) ? 0 : p + 1;
   }
   if (MODE == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
