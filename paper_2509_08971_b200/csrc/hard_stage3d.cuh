@@ -7,20 +7,14 @@
 // per-phase activity tests.  Included by hard_kernels.cuh inside namespace hard.
 #pragma once
 
-#ifndef HARD_LDG_POS
-#define HARD_LDG_POS 0
-#endif
 __device__ __forceinline__ double ldg_pinned(const double* p) {
   double v;
   asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
   return v;
 }
 
-#ifndef HARD_SPLIT_BAR
-#define HARD_SPLIT_BAR 1
-#endif
-#ifndef HARD_LATE_FULLBAR
-#define HARD_LATE_FULLBAR 1
+#ifndef HARD_YFIRST_A
+#define HARD_YFIRST_A 1
 #endif
 // Split-phase CTA barrier on an mbarrier (8 arrivals: one elected lane per warp): arrive after producing,
 // wait just before consuming, with independent work in between, so that no warp idles for the slowest one.
@@ -37,6 +31,10 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   constexpr int G = C::G, R = C::R, TX = C::TX, TY = C::TY, BX = C::BX, VS = C::VS, SLOT = C::SLOT, NS = C::NS,
                 NYI = C::NYI;
   constexpr bool LATE = (R >= 2);          // no spare ring slot: the next plane is requested after the z reconstruction
+  // phase order after the y reconstruction: y fluxes then x (frees the y plus values before the x phase; LATE needs
+  // the full barrier 1 anyway), or x then y fluxes (barrier 1 split-phase around the x phase)
+  constexpr bool YFIRST = HARD_YFIRST_A ? LATE : false;
+  static_assert(YFIRST || !LATE, "the late ring request needs the full barrier of the y-first order");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);
   double* RMy = ring + NS * SLOT;      // y minus values, item-indexed [v][item]
@@ -153,7 +151,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     p = (p + 1 == NS) ? 0 : p + 1;
   }
 
-  uint32_t ph = 0;                                      // phase parity of the two split-phase barriers
+  uint32_t ph = 0;                                      // phase parity of the split-phase barriers
   for (int kk = k0; kk < kend; ++kk) {
     const int znext = kk + 2 + R;
     const bool more = kk + 1 < kend;
@@ -174,39 +172,30 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         for (int v = 0; v < NF; ++v) RMy[v * NYI + tid] = mi[v];
       }
     }
-#if HARD_SPLIT_BAR
-    if (LATE && HARD_LATE_FULLBAR) {
-      __syncthreads();                                 // the oldest plane is free once every warp is past its z reconstruction
-      if (more && tid == 0) { fence_proxy_async(); issue(znext); }
+    // barrier 1 (RMy written -> read).  YFIRST: a full barrier, the y fluxes follow at once.  Otherwise split-phase:
+    // arrive here, wait before the y fluxes, with the x phase in between.
+    if (YFIRST) {
+      __syncthreads();
+      if (LATE && more && tid == 0) { fence_proxy_async(); issue(znext); }   // every warp is past its z reconstruction
     } else {
-      warp_arrive(barY);                                                         // barrier 1, arrive: RMy written
-      if (LATE && more && tid == 0) {
-        mbar_wait(barY, ph);
-        fence_proxy_async();
-        issue(znext);
-      }
+      warp_arrive(barY);
     }
-#else
-    __syncthreads();                                                             // barrier 1
-    if (LATE && more && tid == 0) { fence_proxy_async(); issue(znext); }
-#endif
-
-    // own-cell conserved values for the RK combination (consumed after barrier 2), requested here so that the
-    // whole x phase covers their latency; volatile asm keeps ptxas from sinking them to the point of use.
+    // own-cell conserved values for the RK combination (consumed in the epilogue), requested early so that a whole
+    // phase covers their latency; volatile asm keeps ptxas from sinking them to the point of use.
     double uc[NF], ua[NF];
     const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
-#if HARD_LDG_POS == 0
-    if (mine) {
+    auto load_own = [&]() {
+      if (mine) {
 #pragma unroll
-      for (int v = 0; v < NF; ++v) uc[v] = ldg_pinned(Usrc + v * g.fstride + pc);
-      if (MODE == MODE_STAGE2) {
+        for (int v = 0; v < NF; ++v) uc[v] = ldg_pinned(Usrc + v * g.fstride + pc);
+        if (MODE == MODE_STAGE2) {
 #pragma unroll
-        for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
+          for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
+        }
       }
-    }
-#endif
+    };
     // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
-    {
+    auto xphase = [&]() {
       double pl[NF], mi[NF], mr[NF], F[NF];
       int o[2 * R + 1];
 #pragma unroll
@@ -220,12 +209,9 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         const double Fl = __shfl_up_sync(0xffffffffu, F[v], 1, 16);                      // face left of cell tx-1
         Lacc[v] = fma(Fl - F[v], idx, Lacc[v]);
       }
-    }
+    };
     // ---- y fluxes: face above item (between item and item + TX); the top row's result is not used
-#if HARD_SPLIT_BAR
-    if (!(LATE && HARD_LATE_FULLBAR)) mbar_wait(barY, ph);                       // barrier 1, wait: the x phase lay in between
-#endif
-    {
+    auto yflux = [&]() {
       double mr[NF], F[NF];
       const int up = min(tid + TX, NYI - 1);
 #pragma unroll
@@ -235,15 +221,23 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
 #pragma unroll
         for (int v = 0; v < NF; ++v) Fy[v * NYI + tid] = F[v];
       }
+    };
+    // barrier 2 (Fy written -> read) is split-phase in both orders
+    if (YFIRST) {
+      yflux();
+      warp_arrive(barF);
+      load_own();
+      xphase();
+    } else {
+      load_own();
+      xphase();
+      mbar_wait(barY, ph);
+      yflux();
+      warp_arrive(barF);
+      if (more) wait_convert(znext);                   // independent of Fy: covers the other warps' arrival
     }
-#if HARD_SPLIT_BAR
-    warp_arrive(barF);                                                           // barrier 2, arrive: Fy written
-    if (more) wait_convert(znext);                     // independent of Fy: covers the other warps' arrival
-    mbar_wait(barF, ph);                                                         // barrier 2, wait
+    mbar_wait(barF, ph);
     ph ^= 1u;
-#else
-    __syncthreads();                                                             // barrier 2
-#endif
 
     // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
     if (mine) {
@@ -261,9 +255,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         if (l < 0.0) bad = 1; else lam_loc = dmax(lam_loc, l);
       }
     }
-#if !HARD_SPLIT_BAR
-    if (more) wait_convert(znext);
-#endif
+    if (YFIRST && more) wait_convert(znext);
     p = (p + 1 == NS) ? 0 : p + 1;
   }
   if (MODE == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
