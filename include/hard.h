@@ -121,10 +121,16 @@ int hard_lambda_ptr(hard_ctx*, int next, double** dev_ptr);
 /* HARD_VARIANT_*; may be switched at any time between steps (same state buffers). */
 int hard_set_variant(hard_ctx*, int variant);
 
-/* cudaStream_t to enqueue on (e.g. torch.cuda.current_stream().cuda_stream); default stream 0. */
+/* cudaStream_t to enqueue on (e.g. torch.cuda.current_stream().cuda_stream); default stream 0.  On launch-bound
+ * meshes (<= 2^21 cells) hard_step* with >= 8 steps replays a CUDA graph of two steps; the legacy default stream
+ * cannot be captured, so there the library runs those steps on an internal non-blocking stream, ordered after the
+ * work already enqueued on the bound stream and before whatever is enqueued on it next (events, no host sync). */
 int hard_set_stream(hard_ctx*, void* cuda_stream);
 
-/* Bytes of device memory the simulation needs (state buffers + residual + scalar block). */
+/* Bytes of device memory the simulation needs for the variant selected NOW: a 256-B scalar block + two state
+ * buffers (U, U1) for HARD_VARIANT_FUSED, + one more (the residual) for HARD_VARIANT_PERDIR — select the variant
+ * before asking.  If HARD_VARIANT_PERDIR is selected later on a workspace that lacks the third buffer, the library
+ * cudaMalloc's the residual itself on the first per-direction step (HARD_ERR_NOMEM if that fails). */
 size_t hard_workspace_bytes(const hard_ctx*);
 
 /* Lend the library `bytes` >= hard_workspace_bytes() of device memory aligned to 256 B (e.g. a torch
@@ -147,14 +153,17 @@ long long hard_launch_count(const hard_ctx*);
 /* Bracket the stage kernels with CUDA events on the bound stream: after hard_step returns and the
  * stream is synchronised, *ms is the summed device time and *launches the number of stage-kernel
  * launches (fused variant: the fused stage kernel; per-direction variant: all flux/axpy kernels)
- * since the last call with reset != 0.  Used by bench.py for the roofline of the dominant kernel. */
+ * since the last call with reset != 0.  reset = 1 (re)starts the bracketing, reset = 2 stops it (no more events
+ * recorded), reset = 0 only reads.  While it is on, hard_step* does not replay CUDA graphs.  Used by bench.py for
+ * the roofline of the dominant kernel. */
 int hard_stage_time(hard_ctx*, int reset, double* ms, long long* launches);
 
-/* Measurement utility, not on the hot path: fp64 vector peak of the current device in TFLOP/s
- * (register-resident DFMA chains on all SMs, best of 4 timed launches).  BASELINE.md §2 / SURVEY.md
- * Finding 2: the stage kernel is bound by the fp64 pipe, and MEASURED_PEAKS.json has no fp64 entry.
- * The second argument is reserved (may be NULL). */
-int hard_probe_fp64_peak(double* tflops, double* reserved);
+/* ---- environment variables read by the library (tuning / debugging; none is needed for normal use) -------
+ *   HARD_LZ=<n>            planes per z-chunk of the fused stage kernel (default: a cost model, choose_Lz)
+ *   HARD_NO_GRAPH=1        never replay CUDA graphs in hard_step* (launch-bound 1-D meshes then cost more per step)
+ *   HARD_DEBUG_SYNC=1      (read at hard_create) synchronise and check for errors after every kernel launch
+ *   HARD_GENERIC_STAGE=1   3-D meshes use the generic stage kernel instead of the 3-D specialisation (A/B timing)
+ * The fp64-peak probe bench.py uses for its roofline lives in its own library: include/hard_probe.h. */
 
 #ifdef __cplusplus
 }

@@ -41,6 +41,9 @@ struct hard_ctx {
   bool ws_owned = false;
   DevScalars* sc = nullptr;
   double *U = nullptr, *U1 = nullptr, *Rres = nullptr;
+  bool rres_owned = false;          // residual of the per-direction variant cudaMalloc'ed by the library
+  cudaStream_t own_stream = nullptr;   // internal capturable stream for graph replay when the bound stream is the legacy default
+  cudaEvent_t ev_in = nullptr, ev_out = nullptr;
   CUtensorMap tmU, tmU1;
   bool maps_ready = false;
   bool have_state = false;
@@ -56,6 +59,7 @@ struct hard_ctx {
   cudaGraphExec_t gexec = nullptr;
   double g_cfl = 0.0, g_dt = 0.0;
   int g_sig = -1;                   // variant / source / stream signature the graph was captured for
+  long long g_gen = -1, gen = 0;    // generation of everything the captured nodes bake in by value (grid, spacing, source, slab, Lz)
   cudaStream_t g_stream = nullptr;
   bool graphs_ok = true;            // cleared when the bound stream cannot be captured (legacy default stream)
   std::vector<cudaEvent_t> ev;      // start/stop pairs around stage kernels
@@ -125,7 +129,7 @@ void carve(hard_ctx* c) {
   const size_t sb = align_up(state_bytes(c), 256);
   c->U = (double*)p;  p += sb;
   c->U1 = (double*)p; p += sb;
-  c->Rres = (double*)p;
+  if (!c->rres_owned) c->Rres = (c->ws_bytes >= 256 + 3 * sb) ? (double*)p : nullptr;   // else allocated on first use
 }
 
 int make_map(hard_ctx* c, CUtensorMap* m, double* base) {
@@ -296,6 +300,13 @@ int launch_axpy(hard_ctx* c, int stage2, double cfl, double dt_fixed) {
 
 // L(Usrc) into the residual array, one launch per active direction (variant a8)
 int perdir_residual(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, double cfl, double dt_fixed) {
+  if (!c->Rres) {                                          // workspace sized for the fused variant: own residual
+    void* r = nullptr;
+    cudaError_t e = cudaMalloc(&r, state_bytes(c));
+    if (e != cudaSuccess) return fail(c, HARD_ERR_NOMEM, std::string("cudaMalloc (per-direction residual): ") + cudaGetErrorString(e));
+    c->Rres = (double*)r;
+    c->rres_owned = true;
+  }
   int first = 1;
   for (int d = 0; d < 3; ++d) {
     if (!c->g.act[d]) continue;
@@ -334,7 +345,7 @@ bool ensure_graph(hard_ctx* c, double cfl, double dt_fixed) {
   static const bool disabled = getenv("HARD_NO_GRAPH") != nullptr;
   if (disabled || !c->graphs_ok || c->profiling || c->debug_sync || (c->steps_enq & 1)) return false;
   const int sig = c->variant * 4 + (c->src_on ? 2 : 0) + 1;
-  if (c->gexec && c->g_cfl == cfl && c->g_dt == dt_fixed && c->g_sig == sig && c->g_stream == c->stream) return true;
+  if (c->gexec && c->g_cfl == cfl && c->g_dt == dt_fixed && c->g_sig == sig && c->g_stream == c->stream && c->g_gen == c->gen) return true;
   if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
   if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
     cudaGetLastError();
@@ -352,7 +363,7 @@ bool ensure_graph(hard_ctx* c, double cfl, double dt_fixed) {
   e = cudaGraphInstantiate(&c->gexec, graph, 0);
   cudaGraphDestroy(graph);
   if (e != cudaSuccess) { cudaGetLastError(); c->gexec = nullptr; c->graphs_ok = false; return false; }
-  c->g_cfl = cfl; c->g_dt = dt_fixed; c->g_sig = sig; c->g_stream = c->stream;
+  c->g_cfl = cfl; c->g_dt = dt_fixed; c->g_sig = sig; c->g_stream = c->stream; c->g_gen = c->gen;
   return true;
 }
 
@@ -361,15 +372,46 @@ int do_steps(hard_ctx* c, double cfl, double dt_fixed, int nsteps) {
   int rc = ensure_ready(c);
   if (rc) return rc;
   int left = nsteps;
-  if (left >= 8 && c->stream != 0 && c->variant == HARD_VARIANT_FUSED) {
+  const long long cells = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2];
+  const bool want_graph = left >= 8 && c->variant == HARD_VARIANT_FUSED && c->graphs_ok && !c->profiling && !c->debug_sync;
+  // The legacy default stream cannot be captured: launch-bound meshes borrow an internal non-blocking stream,
+  // ordered after the bound stream's earlier work and before its later work by two events.
+  cudaStream_t user = c->stream;
+  bool borrowed = false;
+  if (want_graph && user == 0 && cells <= (1LL << 21)) {
+    if (!c->own_stream) {
+      if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+          cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        c->own_stream = nullptr;
+      }
+    }
+    if (c->own_stream) {
+      CK(cudaEventRecord(c->ev_in, user));
+      CK(cudaStreamWaitEvent(c->own_stream, c->ev_in, 0));
+      c->stream = c->own_stream;
+      borrowed = true;
+    }
+  }
+  auto give_back = [&](int code) {
+    if (borrowed) {
+      c->stream = user;
+      if (cudaEventRecord(c->ev_out, c->own_stream) != cudaSuccess || cudaStreamWaitEvent(user, c->ev_out, 0) != cudaSuccess)
+        return code ? code : cuda_fail(c, cudaGetLastError(), "internal stream hand-back");
+    }
+    return code;
+  };
+  if (want_graph && c->stream != 0) {
     if (c->steps_enq & 1) {                              // the captured pair starts on an even step
-      if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return rc;
+      if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return give_back(rc);
       --left;
     }
     if (ensure_graph(c, cfl, dt_fixed)) {
       const long long per_pair = 8 + (c->src_on ? 2 : 0);
       while (left >= 2) {
-        CK(cudaGraphLaunch(c->gexec, c->stream));
+        cudaError_t e = cudaGraphLaunch(c->gexec, c->stream);
+        if (e != cudaSuccess) return give_back(cuda_fail(c, e, "cudaGraphLaunch"));
         c->steps_enq += 2;
         c->launches += per_pair;
         left -= 2;
@@ -377,8 +419,8 @@ int do_steps(hard_ctx* c, double cfl, double dt_fixed, int nsteps) {
     }
   }
   for (; left > 0; --left)
-    if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return rc;
-  return HARD_OK;
+    if ((rc = enqueue_one_step(c, cfl, dt_fixed))) return give_back(rc);
+  return give_back(HARD_OK);
 }
 
 int sync_status(hard_ctx* c, DevScalars* host) {
@@ -451,6 +493,10 @@ int hard_destroy(hard_ctx* c) {
   cudaStreamSynchronize(c->stream);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   if (c->gexec) cudaGraphExecDestroy(c->gexec);
+  if (c->own_stream) { cudaStreamSynchronize(c->own_stream); cudaStreamDestroy(c->own_stream); }
+  if (c->ev_in) cudaEventDestroy(c->ev_in);
+  if (c->ev_out) cudaEventDestroy(c->ev_out);
+  if (c->rres_owned && c->Rres) cudaFree(c->Rres);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
   delete c;
   return HARD_OK;
@@ -464,6 +510,7 @@ int hard_set_spacing(hard_ctx* c, double dx, double dy, double dz) {
   DeviceGuard dg__(c);
   if (!c || !(dx > 0.0 && dy > 0.0 && dz > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_spacing: spacings must be > 0");
   c->g.inv_d[0] = 1.0 / dx; c->g.inv_d[1] = 1.0 / dy; c->g.inv_d[2] = 1.0 / dz;
+  c->gen++;                                              // a captured graph holds the old spacing by value
   if (c->have_state) {
     const int slot = (int)(c->steps_enq & 1);
     CK(cudaMemsetAsync(&c->sc->lam_bits[slot], 0, sizeof(unsigned long long), c->stream));
@@ -513,6 +560,7 @@ int hard_set_source(hard_ctx* c, double kappa, double c_light, double a_rad, dou
   if (c->nf != 6) return fail(c, HARD_ERR_ARG, "hard_set_source: call hard_enable_radiation first");
   if (!(kappa >= 0.0 && c_light > 0.0 && a_rad > 0.0 && cv > 0.0)) return fail(c, HARD_ERR_ARG, "hard_set_source: bad parameter");
   c->src_on = true;
+  c->gen++;
   c->src.kappa = kappa; c->src.c_light = c_light; c->src.a_rad = a_rad; c->src.cv = cv;
   return HARD_OK;
 }
@@ -522,6 +570,7 @@ int hard_set_slab(hard_ctx* c, int lower_neighbor, int upper_neighbor) {
   if (!c->g.act[2]) return fail(c, HARD_ERR_ARG, "hard_set_slab: the z direction is inactive");
   c->zskip = (lower_neighbor ? 1 : 0) | (upper_neighbor ? 2 : 0);
   c->g.zskip = c->zskip;
+  c->gen++;
   return HARD_OK;
 }
 
@@ -589,7 +638,7 @@ int hard_set_stream(hard_ctx* c, void* s) {
 
 size_t hard_workspace_bytes(const hard_ctx* c) {
   if (!c) return 0;
-  return 256 + 3 * align_up(state_bytes(c), 256);
+  return 256 + (c->variant == HARD_VARIANT_PERDIR ? 3 : 2) * align_up(state_bytes(c), 256);
 }
 
 int hard_bind_workspace(hard_ctx* c, void* dev, size_t bytes) {
@@ -619,6 +668,7 @@ int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const doubl
   if (c->nf == 6) CK(cudaMemsetAsync(c->U + 5 * c->g.fstride, 0, (size_t)c->g.fstride * sizeof(double), c->stream));
   CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
   c->steps_enq = 0;
+  c->gen++;
   c->have_state = true;
   c->err.clear();
   if ((rc = launch_cfl(c, c->U, 0))) return rc;
@@ -685,7 +735,7 @@ int hard_stage_time(hard_ctx* c, int reset, double* ms, long long* launches) {
   }
   if (ms) *ms = tot;
   if (launches) *launches = (long long)(c->ev_used / 2);
-  if (reset) { c->ev_used = 0; c->profiling = true; }
+  if (reset) { c->ev_used = 0; c->profiling = (reset == 1); }
   return HARD_OK;
 }
 

@@ -337,7 +337,7 @@ struct StageCfg {
 // state reconstructs.
 template <int S, int NF>
 __device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double* pl, double* mi) {
-  constexpr int R = SchemeTraits<S>::R, VS = StageCfg<S, NF>::VS;
+  constexpr int VS = StageCfg<S, NF>::VS;
   if (S == SCHEME_A) {
     double c[NF], wp[NF], wm[NF];
     constexpr int order[6] = { 0, 4, 1, 2, 3, 5 };       // rho and p first: they decide the fallback

@@ -1,9 +1,11 @@
-// hard_probe.cu — measurement utility (not on the hot path): register-resident DFMA chains on every
+// hard_probe.cu — measurement utility (not on the hot path; its own library libhard_probe.so, include/hard_probe.h): register-resident DFMA chains on every
 // SM, to measure the fp64 vector peak that bounds the stage kernel (MEASURED_PEAKS.json has no fp64
 // entry; BASELINE.md §2 asks for this measurement).
 #include <cuda_runtime.h>
 
-#include "../../include/hard.h"
+#include "../../include/hard_probe.h"
+
+enum { HARD_OK = 0, HARD_ERR_ARG = -1, HARD_ERR_CUDA = -2, HARD_ERR_NOMEM = -3 };   // the codes of include/hard.h
 
 namespace {
 __global__ void __launch_bounds__(256) dfma_chain_kernel(double* out, int iters, double a, double b) {

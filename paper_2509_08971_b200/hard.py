@@ -13,6 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libhard_b200.so")
+PROBE_LIB_PATH = os.path.join(_HERE, "libhard_probe.so")     # include/hard_probe.h: measurement utility, not the product ABI
 
 OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_NOSTATE, ERR_NONPHYSICAL = 0, -1, -2, -3, -4, -5
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT = 0, 1, 2
@@ -22,7 +23,7 @@ VARIANT_FUSED, VARIANT_PERDIR = 0, 1
 EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard_max_dt", "hard_destroy",
            "hard_set_spacing", "hard_set_scheme", "hard_set_variant", "hard_set_stream", "hard_workspace_bytes",
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
-           "hard_stage_time", "hard_probe_fp64_peak", "hard_enable_radiation", "hard_set_rad_energy",
+           "hard_stage_time", "hard_enable_radiation", "hard_set_rad_energy",
            "hard_get_rad_energy", "hard_set_source", "hard_set_slab", "hard_halo_doubles", "hard_halo_pack",
            "hard_halo_unpack", "hard_substep", "hard_lambda_ptr"]
 
@@ -75,15 +76,24 @@ def lib():
     L.hard_halo_unpack.argtypes = [vp, c_int, c_int, dp]
     L.hard_substep.argtypes = [vp, c_dbl, c_dbl, c_int]
     L.hard_lambda_ptr.argtypes = [vp, c_int, ctypes.POINTER(ctypes.c_void_p)]
-    L.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(c_dbl), ctypes.POINTER(c_dbl)]
     _lib = L
     return L
 
 
+_probe = None
+
+
 def probe_fp64_peak():
-    """fp64 vector peak of the current device, TFLOP/s (measurement utility)."""
+    """fp64 vector peak of the current device, TFLOP/s (measurement utility, libhard_probe.so)."""
+    global _probe
+    if _probe is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            from . import build as _build
+            _build.build()
+        _probe = ctypes.CDLL(PROBE_LIB_PATH)
+        _probe.hard_probe_fp64_peak.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     v = ctypes.c_double()
-    rc = lib().hard_probe_fp64_peak(ctypes.byref(v), None)
+    rc = _probe.hard_probe_fp64_peak(ctypes.byref(v), None)
     if rc != OK:
         raise HardError(rc, "hard_probe_fp64_peak")
     return v.value
@@ -224,7 +234,12 @@ class Hard:
         return int(self.L.hard_workspace_bytes(self.h))
 
     def run_to(self, t_end, cfl, max_steps=10 ** 7):
-        """Harness loop: hard_step(cfl, 1) while t < t_end, last step clamped."""
+        """Harness loop: hard_step(cfl, .) while t < t_end, last step clamped to land on t_end.
+
+        Far from t_end the steps are enqueued in batches (one host synchronisation per batch instead of two per
+        step; on launch-bound meshes the batch replays a CUDA graph): a batch covers at most a quarter of the
+        remaining time at the current dt, so it cannot reach t_end unless dt quadruples inside it — checked.
+        The dt sequence is the same as stepping one by one: dt_n = cfl / lambda(U^n) is evaluated on the device."""
         n = 0
         while n < max_steps:
             t, _ = self.time()
@@ -235,6 +250,14 @@ class Hard:
                 self.step_dt(t_end - t, 1)
                 n += 1
                 break
-            self.step(cfl, 1)
-            n += 1
+            batch = min(int(0.25 * (t_end - t) / dt), max_steps - n, 4096)
+            if batch >= 8:
+                self.step(cfl, batch)
+                n += batch
+                t2, _ = self.time()
+                if t2 >= t_end:
+                    raise HardError(ERR_ARG, "run_to: a batch of steps overshot t_end (dt grew more than fourfold)")
+            else:
+                self.step(cfl, 1)
+                n += 1
         return n

@@ -30,6 +30,34 @@ def test_library_builds_and_exports_every_declared_symbol():
     out = subprocess.run(["nm", "-D", "--defined-only", hard.LIB_PATH], capture_output=True, text=True).stdout
     for name in decl:
         assert re.search(r"\sT\s+%s$" % name, out, flags=re.M), name
+    # the fp64-peak probe is a separate library with its own header: not part of the product ABI
+    assert "hard_probe_fp64_peak" not in out
+    pout = subprocess.run(["nm", "-D", "--defined-only", hard.PROBE_LIB_PATH], capture_output=True, text=True).stdout
+    assert re.search(r"\sT\s+hard_probe_fp64_peak$", pout, flags=re.M)
+    assert "hard_probe_fp64_peak" in open(os.path.join(ROOT, "include", "hard_probe.h")).read()
+
+
+def build_cabi_program():
+    """gcc tests/test_cabi.c -I include against libhard_b200.so -> tests/test_cabi (plain C, no Python in the loop)."""
+    from paper_2509_08971_b200 import build, hard
+    build.build()
+    exe = os.path.join(ROOT, "tests", "test_cabi.bin")
+    libdir = os.path.dirname(hard.LIB_PATH)
+    cmd = ["gcc", "-std=c99", "-Wall", "-Werror", "-O1", "-I", os.path.join(ROOT, "include"),
+           os.path.join(ROOT, "tests", "test_cabi.c"), "-o", exe, "-L", libdir, "-lhard_b200",
+           "-Wl,-rpath," + libdir, "-lm"]
+    subprocess.check_call(cmd)
+    return exe
+
+
+def test_c_program_compiles_against_the_header():
+    # SURVEY §8(b): the boundary is a C ABI — a C99 compiler accepts include/hard.h as it stands and the five
+    # north-star calls link; the program itself runs on the GPU box (tests/test_gpu_api.py::test_cabi_c_program)
+    exe = build_cabi_program()
+    assert os.path.exists(exe)
+    syms = subprocess.run(["nm", "-D", "--undefined-only", exe], capture_output=True, text=True).stdout
+    for name in ("hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard_max_dt"):
+        assert name in syms
 
 
 def test_sass_contains_tma_and_fp64_pipe_instructions():

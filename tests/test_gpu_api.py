@@ -91,7 +91,7 @@ def test_non_default_stream_and_library_owned_workspace():
     assert max(field_errors(out, ref)) <= 1e-11
     h.close()
     h2 = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing, torch_workspace=False)   # cudaMalloc'ed by the library
-    assert h2.workspace_bytes() > 3 * 5 * 20 ** 3 * 8
+    assert 2 * 5 * 20 ** 3 * 8 < h2.workspace_bytes() < 3 * 5 * 26 ** 3 * 8   # fused: scalar block + U + U1
     h2.set_state(*w.state)
     h2.step(w.cfl, 3)
     assert max(field_errors(h2.get_state(), ref)) <= 1e-11
@@ -175,11 +175,12 @@ def test_graph_replay_on_a_capturable_stream_matches_direct_launches(scheme):
     configs); the result must equal the directly launched run bit for bit, for even and odd step counts."""
     import torch
     w = wl.sod(1000)
-    ref = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)     # default stream: direct launches
+    ref = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)     # one step per call: direct launches
     ref.set_state(*w.state)
-    ref.step(w.cfl, 3)
-    ref.step(w.cfl, 25)
-    ref.step_dt(1e-5, 9)
+    for _ in range(28):
+        ref.step(w.cfl, 1)
+    for _ in range(9):
+        ref.step_dt(1e-5, 1)
     exp, t_exp = ref.get_state(), ref.time()
     n_direct = ref.launch_count()
     ref.close()
@@ -196,3 +197,93 @@ def test_graph_replay_on_a_capturable_stream_matches_direct_launches(scheme):
         assert np.array_equal(a, b)
     assert t_out == t_exp
     h.close()
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_graph_is_recaptured_when_spacing_or_state_changes(scheme):
+    """the captured kernel nodes hold the grid descriptor (1/dx, slab flags), the source parameters and
+    Lz by value; hard_set_spacing / hard_set_source / hard_set_slab / hard_set_state must invalidate the graph."""
+    import torch
+    w = wl.sod(400)
+    sp2 = (2.0 * w.spacing[0], 1.0, 1.0)
+
+    def run(batched):
+        h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+        h.set_state(*w.state)
+        for spacing in (None, sp2, w.spacing):
+            if spacing is not None:
+                h._chk(h.L.hard_set_spacing(h.h, *spacing))
+            if batched:
+                h.step(w.cfl, 10)                        # >= 8: captured graph, replayed
+            else:
+                for _ in range(10):
+                    h.step(w.cfl, 1)                     # direct launches
+        out, t = h.get_state(), h.time()
+        h.close()
+        return out, t
+
+    exp, t_exp = run(False)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        out, t_out = run(True)
+    for a, b in zip(out, exp):
+        assert np.array_equal(a, b)
+    assert t_out == t_exp
+    out, t_out = run(True)                               # default stream: internal capturable stream
+    for a, b in zip(out, exp):
+        assert np.array_equal(a, b)
+    assert t_out == t_exp
+
+
+def test_default_stream_batches_are_ordered_with_the_callers_stream():
+    """Launch-bound meshes replay graphs on an internal non-blocking stream when the bound stream is the legacy
+    default stream; work enqueued on the default stream before / after must still be ordered before / after."""
+    import torch
+    w = wl.sod(512)
+    h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing, stream=0)
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in w.state]
+    scaled = [a * 1.0 for a in dev]                      # produced on the default stream just before set_state
+    h.set_state(*scaled)
+    h.step(w.cfl, 40)
+    out = [torch.empty_like(a) for a in dev]
+    h.get_state(out)                                     # device-to-device on the bound (default) stream
+    total = sum(float(a.sum()) for a in out)             # consumed on the default stream right after
+    ref = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)
+    ref.set_state(*w.state)
+    for _ in range(40):
+        ref.step(w.cfl, 1)
+    exp = ref.get_state()
+    for a, b in zip(out, exp):
+        assert np.array_equal(a.cpu().numpy(), b)
+    assert total == pytest.approx(sum(float(b.sum()) for b in exp), rel=1e-13)
+    assert h.launch_count() == ref.launch_count()
+    h.close()
+    ref.close()
+
+
+def test_stage_time_can_be_switched_off_and_residual_is_allocated_on_demand():
+    w = wl.turbulence(24, nsteps=2)
+    ref, _ = _oracle_run(w, 0, 4)
+    h = hard.Hard(*w.n, w.gamma, w.bc, spacing=w.spacing)          # workspace sized for the fused variant
+    fused_bytes = h.workspace_bytes()
+    h.set_state(*w.state)
+    h.stage_time(reset=1)
+    h.step(w.cfl, 1)
+    assert h.stage_time(reset=2)[1] == 2                            # two stage launches bracketed; bracketing now off
+    h.step(w.cfl, 1)
+    assert h.stage_time(reset=0)[1] == 0                            # nothing recorded since
+    h.set_variant(hard.VARIANT_PERDIR)                              # no third buffer in the bound workspace
+    assert h.workspace_bytes() > fused_bytes                        # what a per-direction workspace would need
+    h.step(w.cfl, 2)                                                # the library allocates the residual itself
+    assert max(field_errors(h.get_state(), ref)) <= 1e-11
+    h.close()
+
+
+def test_cabi_c_program():
+    """tests/test_cabi.c: plain C against include/hard.h, the five north-star calls on Sod-64 with hand values."""
+    import subprocess
+    from test_boundary_cpu import build_cabi_program
+    exe = build_cabi_program()
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "test_cabi ok" in out.stdout
