@@ -3,6 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
                   [--workload c4|c3|c2s] [--scheme A|B] [--variant fused|perdir]
+                  [--no-e2e] [--no-cpu-baseline] [--no-variants] [--no-ncu-traffic]
 
 One "step" = one Heun / SSP-RK2 step of the whole hot path (ghost fill, stage 1, ghost fill, stage 2
 with the fused CFL reduction) over the workload's full mesh.  Metric (BASELINE.json): fp64 cell-updates
@@ -29,12 +30,12 @@ METRIC = "fp64 cell-updates/sec per RK stage"
 UNIT = "cell-stage-updates/s"
 ALG_BYTES_PER_CELL_STAGE = 100.0     # stage 1 = 40 R + 40 W, stage 2 = 80 R + 40 W  => 100 B average
 # hand count of the method's minimal fp64 operations per cell-stage (1 FMA = 2 flop)
-# (A: 1300, B: 540 fp64-pipe instructions; 2 flop-equivalents each, the DFMA peak's own unit)
+# (A: 1300, B: 540 fp64-pipe instructions; 2 flop-equivalents each, the DFMA peak's own unit).  This is the round-1
+# count and it is kept fixed as the unit of work: it is LOWER than SURVEY.md §8(d)'s table (1 700-1 900 / 520-650
+# instructions, i.e. 3 400-3 800 / 1 040-1 300 in this unit), hence the conservative choice, and ncu's executed
+# counts back it (profiles/README.md).  A kernel that needs fewer instructions than this for the same update
+# raises `frac` legitimately.
 ALG_FLOP_PER_CELL_STAGE = {"A": 2600.0, "B": 1080.0}
-
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-1 launch at 896^3 from the committed ncu capture
-# (profiles/stage_A_r1_v5_ncu.txt, stage_B_r1_v5_ncu.txt); algorithmic bytes of that launch: 80 B x 896^3 = 57.5e9
-NCU_TRAFFIC_STAGE1_C4 = {"A": 37.268129e9 + 28.982001e9, "B": 34.111760e9 + 28.935036e9}
 
 WORKLOADS = {"c4": (896, 10), "c3": (512, 20), "c2s": (256, 10)}
 
@@ -53,6 +54,10 @@ def parse():
                     help="N > 1: split ONE mesh into z-slabs with halo exchange (NEXT-4, strong scaling) instead of replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the short extra measurements of the per-direction variant and of the other scheme")
+    ap.add_argument("--no-ncu-traffic", action="store_true",
+                    help="do not measure roofline.traffic (DRAM bytes of the stage kernel) with an ncu child run")
     return ap.parse_args()
 
 
@@ -157,6 +162,54 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------ DRAM traffic (ncu child run)
+def ncu_stage_traffic(args, timeout=240):
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per stage-kernel launch, measured by running
+    this same bench (2 steps, nothing else) as a child under ncu and averaging the stage-1 and stage-2 launches of
+    the second step.  Only the byte counters come from the profiled run — never a time.  None if ncu is missing,
+    closed on the pool, or the child fails."""
+    import shutil
+    import signal
+    import tempfile
+    ncu = shutil.which("ncu") or "/usr/local/cuda/bin/ncu"
+    if not os.path.exists(ncu):
+        return None, "ncu not found"
+    log = tempfile.NamedTemporaryFile(prefix="hard_ncu_", suffix=".csv", delete=False).name
+    cmd = [ncu, "--metrics", "dram__bytes_read.sum,dram__bytes_write.sum", "--clock-control", "none", "--print-units", "base",
+           "-k", "regex:stage", "-s", "2", "-c", "2", "--csv", "--log-file", log,
+           sys.executable, os.path.abspath(__file__), "--workload", args.workload, "--scheme", args.scheme,
+           "--variant", "fused", "--steps", "2", "--warmup", "0", "--no-e2e", "--no-cpu-baseline", "--no-variants",
+           "--no-ncu-traffic"] + (["--radiation"] if args.radiation else [])
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK=os.environ.get("LOCAL_RANK", "0"))
+    try:
+        p = subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, env=env, start_new_session=True)
+        try:
+            out, _ = p.communicate(timeout=timeout)
+        except subprocess.TimeoutExpired:
+            os.killpg(p.pid, signal.SIGKILL)
+            return None, "ncu child run timed out"
+        if p.returncode != 0:
+            return None, "ncu child run failed: " + (out or "").strip().splitlines()[-1][:160] if out else "ncu child run failed"
+        import csv
+        rows = [r for r in csv.reader(open(log)) if len(r) > 6]
+        H = rows[0]
+        per_launch = {}
+        for r in rows[1:]:
+            d = dict(zip(H, r))
+            per_launch.setdefault(d["ID"], 0.0)
+            per_launch[d["ID"]] += float(d["Metric Value"].replace(",", ""))
+        if len(per_launch) != 2:
+            return None, "ncu child run captured %d stage launches, expected 2" % len(per_launch)
+        return sum(per_launch.values()) / 2.0, "measured in this run: " + " ".join(cmd[:13]) + " ... (child bench, 2 steps)"
+    except Exception as ex:
+        return None, "ncu child run: %s" % str(ex)[:160]
+    finally:
+        try:
+            os.unlink(log)
+        except OSError:
+            pass
+
+
 # ------------------------------------------------------------------------------------ CUDA arm
 def run_cuda(args):
     import torch
@@ -250,9 +303,9 @@ def run_cuda(args):
     alg_tflops = cell_stages_per_launch * ALG_FLOP_PER_CELL_STAGE[args.scheme] / (per_launch_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "stage_kernel<%s>" % args.scheme, "achieved": alg_tflops, "peak": fp64_peak,
                 "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None,
-                "traffic": NCU_TRAFFIC_STAGE1_C4[args.scheme] if (args.workload == "c4" and variant == hard.VARIANT_FUSED) else None,
-                "traffic_note": "ncu dram bytes of one stage-1 launch (algorithmic: 80 B/cell = 57.5e9); profiles/stage_*_r1_v5_ncu.txt",
-                "peak_source": "measured live: hard_probe_fp64_peak (DFMA chains, all SMs)",
+                "traffic": None, "traffic_note": "not measured in this run",
+                "alg_bytes_per_launch": slab_cells * alg_bytes,
+                "peak_source": "measured live: hard_probe_fp64_peak (DFMA chains on all SMs, libhard_probe.so)",
                 "avg_launch_ms": per_launch_ms, "launches_timed": stage_launches,
                 "alg_flop_per_cell_stage": ALG_FLOP_PER_CELL_STAGE[args.scheme]}
     roofline_hbm = {"bound": "hbm", "achieved": alg_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": alg_gbs / hbm_peak,
@@ -292,6 +345,47 @@ def run_cuda(args):
         except Exception as ex:                      # e.g. not enough pinned host memory on the box
             e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
     h.close()
+    del h
+    w.state = None
+    torch.cuda.empty_cache()
+
+    # ---- short side measurements in the same run (BASELINE.json configs[4]: "fused vs per-direction kernels"):
+    # the per-direction variant of this scheme and the fused kernel of the other scheme, device-resident, CUDA events
+    variants = None
+    if rank == 0 and world == 1 and not args.no_variants and not args.radiation and variant == hard.VARIANT_FUSED:
+        variants = {}
+        other = "B" if args.scheme == "A" else "A"
+        for name, sch, var, k in (("perdir_" + args.scheme, args.scheme, hard.VARIANT_PERDIR, 3),
+                                  ("fused_" + other, other, hard.VARIANT_FUSED, max(3, K // 2))):
+            try:
+                wv = wl.turbulence(n, nsteps=k, device=dev)
+                hv = hard.Hard(*wv.n, wv.gamma, wv.bc, scheme=hard.SCHEME_WENO5Z_HLL if sch == "A" else hard.SCHEME_MUSCL_HLLC,
+                               variant=var, spacing=wv.spacing)
+                hv.set_state(*wv.state)
+                hv.step(wv.cfl, 1)
+                hv.set_state(*wv.state)
+                l0 = hv.launch_count()
+                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                ev0.record(stream)
+                hv.step(wv.cfl, k)
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                msv = ev0.elapsed_time(ev1)
+                hv.time()                                  # surfaces a latched non-physical state
+                variants[name] = {"value": cells * 2.0 * k / (msv * 1e-3), "unit": UNIT, "steps": k, "warmup": 1,
+                                  "ms_per_step": msv / k, "gpu_launches": hv.launch_count() - l0,
+                                  "alg_GBs": cells * 200.0 * k / (msv * 1e-3) / 1e9}
+                hv.close()
+                del hv, wv
+                torch.cuda.empty_cache()
+            except Exception as ex:
+                variants[name] = {"value": None, "error": str(ex)[:200]}
+
+    if rank == 0 and world == 1 and not args.no_ncu_traffic and variant == hard.VARIANT_FUSED and not shard:
+        traffic, note = ncu_stage_traffic(args)
+        roofline["traffic"] = traffic
+        roofline["traffic_note"] = note + "; average of one stage-1 and one stage-2 launch; algorithmic bytes per launch in alg_bytes_per_launch"
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -310,7 +404,7 @@ def run_cuda(args):
                            "l2": "state (%.1f GB per buffer) is far larger than the 126 MB L2; no flush needed" % (5 * cells * 8 / 1e9),
                            "sim_time": t_sim, "steps_done": steps_done},
                 "roofline": roofline, "roofline_hbm": roofline_hbm, "e2e": e2e, "cpu_baseline": cpu_baseline,
-                "clocks": clocks, "gpu_launches": launches, "fp64_peak_tflops_measured": fp64_peak}
+                "variants": variants, "clocks": clocks, "gpu_launches": launches, "fp64_peak_tflops_measured": fp64_peak}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
