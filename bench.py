@@ -217,14 +217,29 @@ def run_cuda(args):
     from paper_2509_08971_b200 import hard
     from paper_2509_08971_b200 import workloads as wl
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    has_cuda = torch.cuda.is_available()
+    if has_cuda:
+        torch.cuda.set_device(local)
+    if world > 1:                                  # the communicator comes up first (gloo on a box without GPUs)
+        if has_cuda:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
+    if not has_cuda:
+        msg = "bench.py: no CUDA device; the CUDA path has no CPU fallback"
+        if world > 1:
+            from paper_2509_08971_b200 import sharded
+            comm = sharded.DistComm(True)          # the z-slab neighbour map and pairing code of --shard
+            dist.barrier()
+            msg += " (communicator up: world %d, backend %s, rank %d, z-slab neighbours %s, slab %s of nz=%d)" % (
+                comm.world, dist.get_backend(), comm.rank, (comm.lo, comm.hi),
+                sharded.split_z(WORKLOADS[args.workload][0], world)[rank], WORKLOADS[args.workload][0])
+            dist.destroy_process_group()
+        print(msg, file=sys.stderr, flush=True)
+        raise SystemExit(3)
     dev = torch.device("cuda", local)
 
     n, _cfg_steps = WORKLOADS[args.workload]

@@ -7,9 +7,12 @@ step the max wavespeed is all-reduced (MAX) in place in the device scalar block,
 same dt on the device: nothing returns to the host inside a step.  All arithmetic stays in the CUDA kernels;
 this module only sequences `hard_substep` phases and the exchanges.
 
-Two communicators implement the same interface: `DistComm` (torch.distributed; NCCL on GPUs, gloo in the CPU
-tests of the exchange logic) and `LocalComm` (several ranks emulated by one process on one GPU: the phases of all
-ranks run in lockstep and halos are copied directly — no kernel ever waits on another rank).
+Communicators with one interface: `DistComm` (torch.distributed on the tensors as they are: NCCL with device
+buffers on GPUs, gloo with host tensors in the CPU tests of the exchange logic), `HostStagedComm` (the same pairing
+code, device buffers staged through pinned host memory — for a backend that cannot move device memory, i.e. gloo:
+this is how the real `ShardedHard` class is exercised with several processes sharing ONE GPU, where NCCL cannot
+run), and `LocalGroup` (several ranks emulated by one process on one GPU: the phases of all ranks run in lockstep
+and halos are copied directly).  In none of them does a kernel wait on another rank.
 """
 from __future__ import annotations
 
@@ -76,6 +79,47 @@ class DistComm:
             self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
 
 
+class HostStagedComm(DistComm):
+    """DistComm for a backend that only moves host memory (gloo): the four halo buffers and the lambda slot are
+    staged through pinned host tensors around the very same send/recv pairing and all-reduce.  The staging copies
+    run on the current CUDA stream, which is synchronised before the host-side exchange and implicitly ordered
+    after it (the copy back is enqueued on the same stream), so the kernels see the halos they would with NCCL."""
+
+    def __init__(self, periodic):
+        super().__init__(periodic)
+        self._host = {}
+
+    def _pinned(self, key, like):
+        import torch
+        t = self._host.get(key)
+        if t is None or t.numel() != like.numel():
+            t = torch.empty(like.numel(), dtype=like.dtype, pin_memory=True)
+            self._host[key] = t
+        return t
+
+    def exchange(self, send_low, send_high, recv_low, recv_high):
+        import torch
+        dev = (send_low, send_high, recv_low, recv_high)
+        host = [self._pinned(k, t) for k, t in zip(("sl", "sh", "rl", "rh"), dev)]
+        host[0].copy_(send_low, non_blocking=True)
+        host[1].copy_(send_high, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        super().exchange(*host)
+        if self.lo is not None:
+            recv_low.copy_(host[2], non_blocking=True)
+        if self.hi is not None:
+            recv_high.copy_(host[3], non_blocking=True)
+
+    def allreduce_max(self, t):
+        import torch
+        if self.world > 1:
+            h = self._pinned("lam", t)
+            h.copy_(t, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+            super().allreduce_max(h)
+            t.copy_(h, non_blocking=True)
+
+
 class Slab:
     """One rank's slab: a `Hard` context over (nx, ny, nz_local) plus its halo buffers."""
 
@@ -129,8 +173,11 @@ class Slab:
 class ShardedHard:
     """One rank of a sharded run (use under torchrun, one process per GPU)."""
 
-    def __init__(self, n, gamma, bc, scheme=hard.SCHEME_WENO5Z_HLL, spacing=None, radiation=False):
-        self.comm = DistComm(bc == hard.BC_PERIODIC)
+    def __init__(self, n, gamma, bc, scheme=hard.SCHEME_WENO5Z_HLL, spacing=None, radiation=False, comm=None):
+        if comm is None:                       # NCCL moves device buffers itself; gloo needs the host staging
+            import torch.distributed as dist
+            comm = (DistComm if dist.get_backend() == "nccl" else HostStagedComm)(bc == hard.BC_PERIODIC)
+        self.comm = comm
         self.slab = Slab(n, gamma, bc, self.comm.rank, self.comm.world, scheme, spacing, radiation)
 
     def set_state(self, fields):
@@ -160,6 +207,9 @@ class ShardedHard:
 
     def max_dt(self):
         return self.slab.h.max_dt()
+
+    def close(self):
+        self.slab.close()
 
 
 class LocalGroup:

@@ -42,28 +42,32 @@ def _subbox(state, lo, size):
     return out
 
 
-def _check_subboxes(n, scheme, boxes, B, device_state, w):
+def _check_subboxes(n, scheme, boxes, B, device_state, w, variant=hard.VARIANT_FUSED):
     """boxes: list of (low corner of the central B^3 cube, steps s)."""
     g = 3 if scheme == hard.SCHEME_WENO5Z_HLL else 2
     smax = max(s for _, s in boxes)
-    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, spacing=w.spacing)
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=scheme, variant=variant, spacing=w.spacing)
     h.set_state(*device_state)
     # the GPU runs hard_step(cfl, 1) per step exactly as bench.py's hard_step(cfl, K) does; dt_i is read back
-    dts, snaps = [], {}
+    dts, got = [], {}
     need = sorted(set(s for _, s in boxes))
     import torch
+    out = [torch.empty_like(a) for a in device_state]          # one reusable full-size read-back buffer
     for i in range(smax):
         dts.append(w.cfl * h.max_dt())
         h.step(w.cfl, 1)
         if i + 1 in need:
-            out = [torch.empty_like(a) for a in device_state]
             h.get_state(out)
-            snaps[i + 1] = out
+            for bi, (lo, s) in enumerate(boxes):
+                if s == i + 1:
+                    got[bi] = _subbox(out, lo, B)
     t, steps = h.time()
     assert steps == smax and abs(t - sum(dts)) <= 1e-13 * t
     h.close()
+    del out
+    torch.cuda.empty_cache()
     worst = 0.0
-    for lo, s in boxes:
+    for bi, (lo, s) in enumerate(boxes):
         m = s * 2 * g
         size = B + 2 * m
         init = _subbox(device_state, [c - m for c in lo], size)
@@ -73,8 +77,7 @@ def _check_subboxes(n, scheme, boxes, B, device_state, w):
             o.step_dt(dts[i], 1)
         ref = [a[m:m + B, m:m + B, m:m + B] for a in o.get_state()]
         o.close()
-        got = _subbox(snaps[s], lo, B)
-        errs = field_errors(got, ref)
+        errs = field_errors(got[bi], ref)
         tol = TOL_1 if s == 1 else TOL_100
         assert max(errs) <= tol, "box %s after %d steps: %s" % (lo, s, errs)
         assert all(np.abs(a - b[m:m + B, m:m + B, m:m + B]).max() > 0 for a, b in zip(ref[:1], init[:1]))
@@ -108,7 +111,8 @@ def _dt0_check(n, scheme, device_state, w):
     assert abs(1.0 / dt_orc - best) <= 1e-12 * best
 
 
-@pytest.mark.parametrize("n,scheme,long_steps,Blong", [(512, hard.SCHEME_WENO5Z_HLL, 10, 16),
+@pytest.mark.parametrize("n,scheme,long_steps,Blong", [(512, hard.SCHEME_WENO5Z_HLL, 20, 8),   # all of configs[3]'s 20 steps:
+                                                      # a (8 + 240)^3 oracle block, about six minutes of oracle time
                                                       (512, hard.SCHEME_MUSCL_HLLC, 20, 8),
                                                       (896, hard.SCHEME_WENO5Z_HLL, 10, 16),
                                                       (896, hard.SCHEME_MUSCL_HLLC, 10, 16)])
@@ -126,6 +130,19 @@ def test_throughput_configs_c3_c4_lightcone(n, scheme, long_steps, Blong):
     _check_subboxes(n, scheme, one_step, B, state, w)
     _check_subboxes(n, scheme, [([n - 6, n - 5, n - 7], long_steps)], Blong, state, w)
     del state, w
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("n,scheme", [(896, hard.SCHEME_WENO5Z_HLL), (896, hard.SCHEME_MUSCL_HLLC),
+                                      (512, hard.SCHEME_WENO5Z_HLL)])
+def test_per_direction_variant_c3_c4_lightcone(n, scheme):
+    """BASELINE.json configs[4] compares "fused vs per-direction kernels" at 896^3: the per-direction variant (a8)
+    gets the same light-cone sub-box parity at full size — one step (1e-12) and the config's 10 steps (1e-9)."""
+    import torch
+    w = wl.turbulence(n, device="cuda")
+    boxes = [([n - 10, n - 7, n - 12], 1), ([13 * 14 - 5, 3 * 16 - 9, 224 - 11], 1), ([n - 6, n - 5, n - 7], 10)]
+    _check_subboxes(n, scheme, boxes, 16, w.state, w, variant=hard.VARIANT_PERDIR)
+    del w
     torch.cuda.empty_cache()
 
 

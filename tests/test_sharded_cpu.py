@@ -60,3 +60,24 @@ def test_halo_exchange_and_max_reduction_gloo(tmp_path, world):
     outs = [p.communicate(timeout=300)[0] for p in procs]
     for r, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0 and ("ok %d" % r) in o, o
+
+
+def test_bench_shard_reaches_the_communicator_setup_on_cpu():
+    """`bench.py --shard --gpus 2` launched the way the driver launches it (torchrun, one process per rank): on this
+    GPU-less box the arguments parse, both ranks bring the communicator up (gloo), build the z-slab neighbour map,
+    and only then stop because there is no CUDA device (exit code 3, no CPU fallback)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("needs a box without a GPU")
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--shard", "--steps", "1", "--warmup", "0"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+    text = out.stdout + out.stderr
+    assert out.returncode != 0
+    for r, nb, slab in ((0, (1, 1), (0, 448)), (1, (0, 0), (448, 896))):
+        assert ("communicator up: world 2, backend gloo, rank %d, z-slab neighbours %s, slab %s of nz=896" % (r, nb, slab)) in text, text[-2000:]
+    assert "no CPU fallback" in text
