@@ -16,6 +16,15 @@ __device__ __forceinline__ double ldg_pinned(const double* p) {
 #ifndef HARD_YFIRST_A
 #define HARD_YFIRST_A 1
 #endif
+#ifndef HARD_LDG_VAR
+#define HARD_LDG_VAR 1
+#endif
+#ifndef HARD_LDG_VARB
+#define HARD_LDG_VARB 0
+#endif
+#ifndef HARD_YFIRST_B
+#define HARD_YFIRST_B 0
+#endif
 // Split-phase CTA barrier on an mbarrier (8 arrivals: one elected lane per warp): arrive after producing,
 // wait just before consuming, with independent work in between, so that no warp idles for the slowest one.
 __device__ __forceinline__ void warp_arrive(uint32_t bar) {
@@ -33,7 +42,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   constexpr bool LATE = (R >= 2);          // no spare ring slot: the next plane is requested after the z reconstruction
   // phase order after the y reconstruction: y fluxes then x (frees the y plus values before the x phase; LATE needs
   // the full barrier 1 anyway), or x then y fluxes (barrier 1 split-phase around the x phase)
-  constexpr bool YFIRST = HARD_YFIRST_A ? LATE : false;
+  constexpr bool YFIRST = LATE ? (HARD_YFIRST_A != 0) : (HARD_YFIRST_B != 0);
   static_assert(YFIRST || !LATE, "the late ring request needs the full barrier of the y-first order");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);
@@ -159,6 +168,23 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     const int slot_c = p * SLOT;                        // plane kk (x/y stencils)
     double Lacc[NF];
     zphase(p, Lacc);
+    // own-cell conserved values for the RK combination (consumed in the epilogue), requested early so that a whole
+    // phase covers their latency; volatile asm keeps ptxas from sinking them to the point of use.
+    double uc[NF], ua[NF];
+    const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
+    auto load_uc = [&]() {
+      if (mine) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) uc[v] = ldg_pinned(Usrc + v * g.fstride + pc);
+      }
+    };
+    auto load_ua = [&]() {
+      if (MODE == MODE_STAGE2 && mine) {
+#pragma unroll
+        for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
+      }
+    };
+    if (!YFIRST && HARD_LDG_VARB == 2) load_uc();
     // ---- y: reconstruct the 14 x 18 items of plane kk; minus values to shared memory
     double plY[NF];
     {
@@ -180,20 +206,6 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     } else {
       warp_arrive(barY);
     }
-    // own-cell conserved values for the RK combination (consumed in the epilogue), requested early so that a whole
-    // phase covers their latency; volatile asm keeps ptxas from sinking them to the point of use.
-    double uc[NF], ua[NF];
-    const long long pc = cell_addr(g, i0 + tx - 1, j0 + ty, kk);
-    auto load_own = [&]() {
-      if (mine) {
-#pragma unroll
-        for (int v = 0; v < NF; ++v) uc[v] = ldg_pinned(Usrc + v * g.fstride + pc);
-        if (MODE == MODE_STAGE2) {
-#pragma unroll
-          for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
-        }
-      }
-    };
     // ---- x: reconstruct cell tx-1 of row ty; neighbours by shuffles inside the 16-lane row segment
     auto xphase = [&]() {
       double pl[NF], mi[NF], mr[NF], F[NF];
@@ -224,12 +236,16 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     };
     // barrier 2 (Fy written -> read) is split-phase in both orders
     if (YFIRST) {
+      if (HARD_LDG_VAR >= 1) load_uc();
+      if (HARD_LDG_VAR == 2) load_ua();
       yflux();
       warp_arrive(barF);
-      load_own();
+      if (HARD_LDG_VAR == 0) load_uc();
+      if (HARD_LDG_VAR <= 1) load_ua();
       xphase();
     } else {
-      load_own();
+      if (HARD_LDG_VARB != 2) load_uc();
+      load_ua();
       xphase();
       mbar_wait(barY, ph);
       yflux();
