@@ -1,10 +1,15 @@
 // hard_stage3d.cuh — the fused RK stage (a2..a7) specialised for the 3-D case: all three directions
-// active, all fluxes in one launch, the stage (1 or 2) a template parameter.  Same tiling, ring, thread
-// mapping and phase order as the generic stage_kernel (hard_kernels.cuh), which keeps serving 1-D / 2-D
-// meshes and the per-direction variant; what the specialisation buys is straight-line code between the
-// two barriers of a plane (ptxas interleaves the serial Riemann chains with the reconstruction of the
-// next phase), loop-carried z state that is updated in place (no register copies at the back edge), and no
-// per-phase activity tests.  Included by hard_kernels.cuh inside namespace hard.
+// active, all fluxes in one launch, the stage (1 or 2) a template parameter.  Same tiling, ring and thread
+// mapping as the generic stage_kernel (hard_kernels.cuh), which keeps serving 1-D / 2-D meshes and the
+// per-direction variant.  What the specialisation buys (measured):
+//  * straight-line code between the synchronisation points of a plane (no activity / mode tests, no ragged-tile
+//    branches: out-of-range lanes recompute a valid item and only the stores are predicated), so ptxas
+//    interleaves the serial Riemann chains with the reconstruction next to them;
+//  * loop-carried z state updated in place (no register copies at the back edge); two peeled lead-in planes;
+//  * split-phase barriers on mbarriers (arrive after producing, wait before consuming) wherever independent work
+//    lies in between: scheme B around the x phase and the plane conversion, scheme A around the x phase;
+//  * own-cell loads for the RK combination pinned early (volatile asm) so a whole phase covers their latency.
+// Included by hard_kernels.cuh inside namespace hard.
 #pragma once
 
 __device__ __forceinline__ double ldg_pinned(const double* p) {
@@ -13,18 +18,6 @@ __device__ __forceinline__ double ldg_pinned(const double* p) {
   return v;
 }
 
-#ifndef HARD_YFIRST_A
-#define HARD_YFIRST_A 1
-#endif
-#ifndef HARD_LDG_VAR
-#define HARD_LDG_VAR 1
-#endif
-#ifndef HARD_LDG_VARB
-#define HARD_LDG_VARB 0
-#endif
-#ifndef HARD_YFIRST_B
-#define HARD_YFIRST_B 0
-#endif
 // Split-phase CTA barrier on an mbarrier (8 arrivals: one elected lane per warp): arrive after producing,
 // wait just before consuming, with independent work in between, so that no warp idles for the slowest one.
 __device__ __forceinline__ void warp_arrive(uint32_t bar) {
@@ -42,7 +35,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   constexpr bool LATE = (R >= 2);          // no spare ring slot: the next plane is requested after the z reconstruction
   // phase order after the y reconstruction: y fluxes then x (frees the y plus values before the x phase; LATE needs
   // the full barrier 1 anyway), or x then y fluxes (barrier 1 split-phase around the x phase)
-  constexpr bool YFIRST = LATE ? (HARD_YFIRST_A != 0) : (HARD_YFIRST_B != 0);
+  constexpr bool YFIRST = LATE;
   static_assert(YFIRST || !LATE, "the late ring request needs the full barrier of the y-first order");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);
@@ -184,7 +177,6 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         for (int v = 0; v < NF; ++v) ua[v] = ldg_pinned(Uaux + v * g.fstride + pc);
       }
     };
-    if (!YFIRST && HARD_LDG_VARB == 2) load_uc();
     // ---- y: reconstruct the 14 x 18 items of plane kk; minus values to shared memory
     double plY[NF];
     {
@@ -236,15 +228,14 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     };
     // barrier 2 (Fy written -> read) is split-phase in both orders
     if (YFIRST) {
-      if (HARD_LDG_VAR >= 1) load_uc();
-      if (HARD_LDG_VAR == 2) load_ua();
+      load_uc();                                       // measured: both requests here, or both after the y fluxes, cost 3-4 %
       yflux();
       warp_arrive(barF);
-      if (HARD_LDG_VAR == 0) load_uc();
-      if (HARD_LDG_VAR <= 1) load_ua();
+      load_ua();
       xphase();
+      if (more) wait_convert(znext);                   // independent of Fy
     } else {
-      if (HARD_LDG_VARB != 2) load_uc();
+      load_uc();
       load_ua();
       xphase();
       mbar_wait(barY, ph);
@@ -271,7 +262,6 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
         if (l < 0.0) bad = 1; else lam_loc = dmax(lam_loc, l);
       }
     }
-    if (YFIRST && more) wait_convert(znext);
     p = (p + 1 == NS) ? 0 : p + 1;
   }
   if (MODE == MODE_STAGE2 && !a.skip_cfl) block_max_to_slot(lam_loc, bad, sc, a.cur ^ 1, red);
