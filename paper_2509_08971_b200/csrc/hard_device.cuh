@@ -74,7 +74,9 @@ __device__ __forceinline__ void wenoz_incr(double a, double b, double c, double 
   const double B1 = fma(s1, s1, fma(k3 * t1, t1, eps));
   const double B2 = fma(s2, s2, fma(k3 * t2, t2, eps));
   const double tau = fabs(B0 - B2);
-  const double X0 = (B0 + tau) * (B1 * B2), X1 = (B1 + tau) * (B0 * B2), X2 = (B2 + tau) * (B0 * B1);
+  // X_k = (B_k + tau) prod_{j != k} B_j = P + tau M_k with M_k = prod_{j != k} B_j, P = B0 B1 B2: 4 DMUL + 3 DFMA
+  const double M0 = B1 * B2, M1 = B0 * B2, M2 = B0 * B1, P = B0 * M0;
+  const double X0 = fma(tau, M0, P), X1 = fma(tau, M1, P), X2 = fma(tau, M2, P);
   const double Y = 6.0 * X1, X0t = 3.0 * X0, X2t = 3.0 * X2;
   const double sp = (X0 + Y) + X2t, sm = (X2 + Y) + X0t;             // 10 x (sum of the unnormalised weights)
   // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
@@ -112,20 +114,23 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
   const double SL = dmin(WL[1] - cL, WR[1] - cR);
   const double SR = dmax(WL[1] + cL, WR[1] + cR);
   alpha = dmax(SR, -SL);                                 // = max(|u_n| + c_s) over the two sides (Rusanov, NEXT-1)
-  if (S == SCHEME_A) {                                   // HLL needs both sides' U and F
+  if (S == SCHEME_A) {
+    // HLL: F = (SR+ F_L - SL- F_R + SL- SR+ (U_R - U_L)) / (SR+ - SL-) = wl G_L - wr G_R with G_L = F_L - SL- U_L,
+    // G_R = F_R - SR+ U_R, wl = SR+ / (SR+ - SL-), wr = SL- / (SR+ - SL-), and SL- = min(SL, 0), SR+ = max(SR, 0):
+    // branch-free, F_L when SL >= 0 and F_R when SR <= 0 (G5's inclusive tie-breaks, to rounding); c > 0 keeps
+    // SR+ - SL- > 0.  With k = rho (u_n - S): G = (k, k u_n + p, k u_t1, k u_t2, E (u_n - S) + p u_n) — the
+    // conserved vector and the physical flux are never formed (12 fp64 instructions fewer per face).
     const double EL = fma(0.5 * WL[0], fma(WL[1], WL[1], fma(WL[2], WL[2], WL[3] * WL[3])), WL[4] * inv_gm1);
     const double ER = fma(0.5 * WR[0], fma(WR[1], WR[1], fma(WR[2], WR[2], WR[3] * WR[3])), WR[4] * inv_gm1);
-    const double UL[5] = { WL[0], WL[0] * WL[1], WL[0] * WL[2], WL[0] * WL[3], EL };
-    const double UR[5] = { WR[0], WR[0] * WR[1], WR[0] * WR[2], WR[0] * WR[3], ER };
-    const double FL[5] = { UL[1], fma(UL[1], WL[1], WL[4]), UL[1] * WL[2], UL[1] * WL[3], (EL + WL[4]) * WL[1] };
-    const double FR[5] = { UR[1], fma(UR[1], WR[1], WR[4]), UR[1] * WR[2], UR[1] * WR[3], (ER + WR[4]) * WR[1] };
-    // Branch-free: with SL- = min(SL, 0), SR+ = max(SR, 0) the HLL formula returns F_L when SL >= 0 and F_R when
-    // SR <= 0 (G5's inclusive tie-breaks, to rounding); c > 0 keeps SR+ - SL- > 0.
     const double SLm = dmin(SL, 0.0), SRp = dmax(SR, 0.0);
+    const double dL = WL[1] - SLm, dR = WR[1] - SRp;
+    const double kL = WL[0] * dL, kR = WR[0] * dR;
+    const double GL[5] = { kL, fma(kL, WL[1], WL[4]), kL * WL[2], kL * WL[3], fma(EL, dL, WL[4] * WL[1]) };
+    const double GR[5] = { kR, fma(kR, WR[1], WR[4]), kR * WR[2], kR * WR[3], fma(ER, dR, WR[4] * WR[1]) };
     const double inv = fast_rcp(SRp - SLm);
-    const double wl = SRp * inv, wr = SLm * inv, ws = wl * SLm;
+    const double wl = SRp * inv, wr = SLm * inv;
 #pragma unroll
-    for (int m = 0; m < 5; ++m) F[m] = fma(ws, UR[m] - UL[m], fma(-wr, FR[m], wl * FL[m]));
+    for (int m = 0; m < 5; ++m) F[m] = fma(-wr, GR[m], wl * GL[m]);
   } else {
     // HLLC, averaged-pressure form (G5).  Only the upwind side's U and F enter the result: side L if
     // SL >= 0 or (SR > 0 and S* > 0), else side R; the supersonic cases return that side's F.

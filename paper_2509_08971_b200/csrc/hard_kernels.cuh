@@ -331,16 +331,18 @@ struct StageCfg {
 
 // Both face values of all five primitives of one cell along one direction; o[s] = ring offset of
 // field 0 at stencil position s - R.  Scheme A applies the positivity fallback (G4): if a reconstructed rho
-// or p is <= 0, all variables of the cell become piecewise constant — done by adding the WENO increments
-// with the factor 0 instead of 1/6, so the fallback costs four extra DFMA and no branch.  "<= 0" is taken on
-// the high words (sign set, or zero): exact for every value but a positive denormal, which no admissible
-// state reconstructs.
+// or p is <= 0, all variables of the cell become piecewise constant.  No branch: rho and p are reconstructed
+// first and fall back by selects; the other variables add their WENO increments with the factor 0 instead of
+// 1/6.  "<= 0" is taken on the high words (sign set, or zero): exact for every value but a positive denormal,
+// which no admissible state reconstructs.
 template <int S, int NF>
 __device__ __forceinline__ void recon_item(const double* __restrict__ ring, const int* o, double* pl, double* mi) {
   constexpr int VS = StageCfg<S, NF>::VS;
   if (S == SCHEME_A) {
     double c[NF], wp[NF], wm[NF];
     constexpr int order[6] = { 0, 4, 1, 2, 3, 5 };       // rho and p first: they decide the fallback
+    // rho and p get their face values at once; if any of the four is <= 0 they fall back to the cell value by
+    // selects (integer pipe), and the other variables take the factor 0 instead of 1/6 in their one DFMA
     int hmin = 0x7fffffff;
     double f6 = 1.0 / 6.0;
 #pragma unroll
@@ -348,12 +350,19 @@ __device__ __forceinline__ void recon_item(const double* __restrict__ ring, cons
       const int v = order[q];
       c[v] = ring[o[2] + v * VS];
       wenoz_incr(ring[o[0] + v * VS], ring[o[1] + v * VS], c[v], ring[o[3] + v * VS], ring[o[4] + v * VS], wp[v], wm[v]);
-      if (q < 2)
-        hmin = min(hmin, min(__double2hiint(fma(wp[v], 1.0 / 6.0, c[v])), __double2hiint(fma(wm[v], 1.0 / 6.0, c[v]))));
-      if (q == 1) f6 = hmin <= 0 ? 0.0 : 1.0 / 6.0;
+      if (q < 2) {
+        pl[v] = fma(wp[v], 1.0 / 6.0, c[v]);
+        mi[v] = fma(wm[v], 1.0 / 6.0, c[v]);
+        hmin = min(hmin, min(__double2hiint(pl[v]), __double2hiint(mi[v])));
+      }
+      if (q == 1) {
+        const bool fb = hmin <= 0;
+        f6 = fb ? 0.0 : 1.0 / 6.0;
+        pl[0] = fb ? c[0] : pl[0]; mi[0] = fb ? c[0] : mi[0];
+        pl[4] = fb ? c[4] : pl[4]; mi[4] = fb ? c[4] : mi[4];
+      }
+      if (q >= 2) { pl[v] = fma(wp[v], f6, c[v]); mi[v] = fma(wm[v], f6, c[v]); }
     }
-#pragma unroll
-    for (int v = 0; v < NF; ++v) { pl[v] = fma(wp[v], f6, c[v]); mi[v] = fma(wm[v], f6, c[v]); }
   } else {
 #pragma unroll
     for (int v = 0; v < NF; ++v)
