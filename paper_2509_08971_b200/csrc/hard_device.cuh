@@ -80,8 +80,9 @@ __device__ __forceinline__ void wenoz_incr(double a, double b, double c, double 
   const double Y = 6.0 * X1, X0t = 3.0 * X0, X2t = 3.0 * X2;
   const double sp = (X0 + Y) + X2t, sm = (X2 + Y) + X0t;             // 10 x (sum of the unnormalised weights)
   // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
-  const double q0 = fma(5.0, d2, -2.0 * d1), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);
-  const double p0 = fma(-5.0, d3, 2.0 * d4), p1 = -fma(2.0, d2, d3), p2 = fma(-4.0, d2, d1);
+  // (5 d2 - 2 d1 = 2 t0 - d2 and 2 d4 - 5 d3 = 2 t2 + d3: one DFMA each)
+  const double q0 = fma(2.0, t0, -d2), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);
+  const double p0 = fma(2.0, t2, d3), p1 = -fma(2.0, d2, d3), p2 = fma(-4.0, d2, d1);
   const double np = fma(X2t, q2, fma(Y, q1, X0 * q0));
   const double nm = fma(X0t, p2, fma(Y, p1, X2 * p0));
   wp = np * fast_rcp(sp);
@@ -119,14 +120,17 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     // G_R = F_R - SR+ U_R, wl = SR+ / (SR+ - SL-), wr = SL- / (SR+ - SL-), and SL- = min(SL, 0), SR+ = max(SR, 0):
     // branch-free, F_L when SL >= 0 and F_R when SR <= 0 (G5's inclusive tie-breaks, to rounding); c > 0 keeps
     // SR+ - SL- > 0.  With k = rho (u_n - S): G = (k, k u_n + p, k u_t1, k u_t2, E (u_n - S) + p u_n) — the
-    // conserved vector and the physical flux are never formed (12 fp64 instructions fewer per face).
-    const double EL = fma(0.5 * WL[0], fma(WL[1], WL[1], fma(WL[2], WL[2], WL[3] * WL[3])), WL[4] * inv_gm1);
-    const double ER = fma(0.5 * WR[0], fma(WR[1], WR[1], fma(WR[2], WR[2], WR[3] * WR[3])), WR[4] * inv_gm1);
+    // conserved vector and the physical flux are never formed (14 fp64 instructions fewer per face).
+    // energy row: E (u_n - S) + p u_n with E = rho |v|^2 / 2 + p / (gamma - 1)  =  (k / 2) |v|^2 + p ((u_n - S) / (gamma - 1) + u_n)
     const double SLm = dmin(SL, 0.0), SRp = dmax(SR, 0.0);
     const double dL = WL[1] - SLm, dR = WR[1] - SRp;
     const double kL = WL[0] * dL, kR = WR[0] * dR;
-    const double GL[5] = { kL, fma(kL, WL[1], WL[4]), kL * WL[2], kL * WL[3], fma(EL, dL, WL[4] * WL[1]) };
-    const double GR[5] = { kR, fma(kR, WR[1], WR[4]), kR * WR[2], kR * WR[3], fma(ER, dR, WR[4] * WR[1]) };
+    const double v2L = fma(WL[1], WL[1], fma(WL[2], WL[2], WL[3] * WL[3]));
+    const double v2R = fma(WR[1], WR[1], fma(WR[2], WR[2], WR[3] * WR[3]));
+    const double GL[5] = { kL, fma(kL, WL[1], WL[4]), kL * WL[2], kL * WL[3],
+                           fma(0.5 * kL, v2L, WL[4] * fma(dL, inv_gm1, WL[1])) };
+    const double GR[5] = { kR, fma(kR, WR[1], WR[4]), kR * WR[2], kR * WR[3],
+                           fma(0.5 * kR, v2R, WR[4] * fma(dR, inv_gm1, WR[1])) };
     const double inv = fast_rcp(SRp - SLm);
     const double wl = SRp * inv, wr = SLm * inv;
 #pragma unroll
