@@ -143,9 +143,10 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     const double Ss = ((WR[4] - WL[4]) + fma(A, WL[1], -B * WR[1])) * fast_rcp(A - B);
     const double pbar = 0.5 * ((WL[4] + WR[4]) + fma(A, Ss - WL[1], B * (Ss - WR[1])));
     // S* lies strictly between SL and SR, so SL >= 0 implies S* > 0 and SR <= 0 implies S* < 0: "left" covers the
-    // supersonic cases too.  F* = F_K + S_K (U*_K - U_K) with U*_K - U_K = (S* U_K - F_K + pbar D*) / (S_K - S*)
-    // — the same flux as the averaged-pressure quotient, regrouped — and S_K clamped to zero on the supersonic
-    // side returns F_K itself: no branch, no select on the result.
+    // supersonic cases too.  With G = F_K - S U_K = (k, k u_n + p, k u_t1, k u_t2, (k/2)|v|^2 + p ((u_n - S)/(gamma-1) + u_n)),
+    // k = rho (u_n - S) (neither U_K nor F_K is formed), the star flux F_K + S_K (U*_K - U_K) with
+    // U*_K = (pbar D* - G) / (S_K - S*), D* = (0, 1, 0, 0, S*), is (1 - g) G + g pbar D*, g = S_K / (S_K - S*).
+    // S clamped to zero on the supersonic side makes G = F_K and g = 0: no branch, no select on the result.
     const bool left = Ss > 0.0;
     double W[5];
 #pragma unroll
@@ -153,17 +154,15 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     const double SK = left ? SL : SR;
     const bool sub = left ? (SK < 0.0) : (SK > 0.0);
     const double SKc = sub ? SK : 0.0;
-    const double E = fma(0.5 * W[0], fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3])), W[4] * inv_gm1);
-    const double UK[5] = { W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E };
-    const double FK[5] = { UK[1], fma(UK[1], W[1], W[4]), UK[1] * W[2], UK[1] * W[3], (E + W[4]) * W[1] };
-    const double g = SKc * fast_rcp(SK - Ss);
-#pragma unroll
-    for (int m = 0; m < 5; ++m) {
-      double t = fma(Ss, UK[m], -FK[m]);
-      if (m == 1) t += pbar;
-      if (m == 4) t = fma(pbar, Ss, t);
-      F[m] = fma(g, t, FK[m]);
-    }
+    const double d = W[1] - SKc, k = W[0] * d;
+    const double v2 = fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3]));
+    const double G4 = fma(0.5 * k, v2, W[4] * fma(d, inv_gm1, W[1]));
+    const double g = SKc * fast_rcp(SK - Ss), h = 1.0 - g, gp = g * pbar;
+    F[0] = h * k;
+    F[1] = fma(h, fma(k, W[1], W[4]), gp);
+    F[2] = h * (k * W[2]);
+    F[3] = h * (k * W[3]);
+    F[4] = fma(h, G4, gp * Ss);
   }
 }
 

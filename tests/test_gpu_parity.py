@@ -174,6 +174,26 @@ def test_radiation_energy_turbulence_100_steps(scheme):
     _check_rad(w, er, scheme, hard.VARIANT_FUSED, 100, TOL_100)
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_radiation_energy_in_cgs_magnitudes(scheme):
+    """Physical-unit data: a stellar-interior-like state in cgs, rho ~ 1e2 g/cm^3, p ~ 1e17 erg/cm^3,
+    v ~ 1e7 cm/s, non-uniform E_rad ~ 1e14..1e15 erg/cm^3, cells of 1e9 cm.  The division-free WENO-Z weights are
+    cubic in the smoothness indicators (data^6 ~ 1e100 here): no overflow, same parity bars."""
+    n = (37, 21, 19)
+    rng = np.random.default_rng(21)
+    shp = n[::-1]
+    rho = 1e2 * (1.0 + 0.3 * rng.random(shp))
+    vel = [1e7 * (rng.random(shp) - 0.5) for _ in range(3)]
+    prs = 1e17 * (1.0 + 0.5 * rng.random(shp))
+    gamma = 5.0 / 3.0
+    E = prs / (gamma - 1.0) + 0.5 * rho * (vel[0] ** 2 + vel[1] ** 2 + vel[2] ** 2)
+    w = wl.Workload("cgs", n, gamma, wl.BC_PERIODIC, (1e9, 0.7e9, 1.3e9), 0.4, nsteps=10,
+                    state=[rho, rho * vel[0], rho * vel[1], rho * vel[2], E])
+    er = 1e14 * (1.0 + 9.0 * rng.random(shp))
+    _check_rad(w, er, scheme, hard.VARIANT_FUSED, 1, TOL_1)
+    _check_rad(w, er, scheme, hard.VARIANT_FUSED, 10, TOL_100)
+
+
 # ---------------------------------------------------------------- NEXT-3: radiative heating / cooling source
 def _check_source(w, er, params, scheme, variant, nsteps, tol, dt=None):
     import oracle
