@@ -321,7 +321,7 @@ def run_cuda(args):
         cell_stages_per_launch = cells * 2.0 * K / max(stage_launches, 1)
     alg_gbs = cell_stages_per_launch * alg_bytes / (per_launch_ms * 1e-3) / 1e9
     alg_tflops = cell_stages_per_launch * ALG_FLOP_PER_CELL_STAGE[args.scheme] / (per_launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "stage_kernel<%s>" % args.scheme, "achieved": alg_tflops, "peak": fp64_peak,
+    roofline = {"bound": "alu", "kernel": ("stage3d_kernel<%s, %d, stage 1|2>" % (args.scheme, nfields)) if variant == hard.VARIANT_FUSED else ("stage_kernel<%s, %d> per direction + axpy_kernel" % (args.scheme, nfields)), "achieved": alg_tflops, "peak": fp64_peak,
                 "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None,
                 "traffic": None, "traffic_note": "not measured in this run",
                 "alg_bytes_per_launch": slab_cells * alg_bytes,
