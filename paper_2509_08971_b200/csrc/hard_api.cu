@@ -201,8 +201,8 @@ int ensure_ready(hard_ctx* c) {
     if (rc) return rc;
 #define HARD_SET_SMEM(S, NF) \
   CK(cudaFuncSetAttribute(stage_kernel<S, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM)); \
-  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM)); \
-  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM));
+  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM3D)); \
+  CK(cudaFuncSetAttribute(stage3d_kernel<S, NF, MODE_STAGE2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)StageCfg<S, NF>::SMEM3D));
     HARD_SET_SMEM(SCHEME_A, 5) HARD_SET_SMEM(SCHEME_B, 5) HARD_SET_SMEM(SCHEME_A, 6) HARD_SET_SMEM(SCHEME_B, 6)
 #undef HARD_SET_SMEM
     c->Lz = choose_Lz(c);
@@ -271,8 +271,8 @@ int launch_stage(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, const d
   const bool spec3d = !generic_only && g.act[0] && g.act[1] && g.act[2] && dirmask == 7 && (mode == MODE_STAGE1 || mode == MODE_STAGE2);
 #define HARD_LAUNCH(S, NF) \
   do { \
-    if (spec3d && mode == MODE_STAGE1) stage3d_kernel<S, NF, MODE_STAGE1><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
-    else if (spec3d) stage3d_kernel<S, NF, MODE_STAGE2><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
+    if (spec3d && mode == MODE_STAGE1) stage3d_kernel<S, NF, MODE_STAGE1><<<grid, 256, StageCfg<S, NF>::SMEM3D, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
+    else if (spec3d) stage3d_kernel<S, NF, MODE_STAGE2><<<grid, 256, StageCfg<S, NF>::SMEM3D, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
     else stage_kernel<S, NF><<<grid, 256, StageCfg<S, NF>::SMEM, c->stream>>>(tm, Usrc, Uaux, Uout, g, c->sc, a); \
   } while (0)
   if (c->scheme == HARD_SCHEME_WENO5Z_HLL) { if (c->nf == 6) HARD_LAUNCH(SCHEME_A, 6); else HARD_LAUNCH(SCHEME_A, 5); }

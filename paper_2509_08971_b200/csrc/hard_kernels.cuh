@@ -325,8 +325,12 @@ struct StageCfg {
   static constexpr int NYI = TX * (TY + 2);                   // y reconstruction items
   static constexpr uint32_t BOX_BYTES = (uint32_t)NF * VS * 8u;
   static constexpr size_t SMEM = (size_t)NS * SLOT * 8 + 2ull * NF * NYI * 8 + NS * 8 + 64 * 8;
+  // stage3d_kernel, scheme B: y items in thread order (hard_stage3d.cuh), exchange arrays of TY+2 rows of pitch BX
+  static constexpr bool YT = (R < 2);
+  static constexpr int NYX = YT ? (TY + 2) * BX : NYI;
+  static constexpr size_t SMEM3D = (size_t)NS * SLOT * 8 + 2ull * NF * NYX * 8 + NS * 8 + 64 * 8;
   // resident CTAs per SM: 2, except WENO with six fields (130 KB of shared memory)
-  static constexpr int CTAS = (SMEM > 113 * 1024) ? 1 : 2;
+  static constexpr int CTAS = (SMEM > 113 * 1024 || SMEM3D > 113 * 1024) ? 1 : 2;
 };
 
 // Both face values of all five primitives of one cell along one direction; o[s] = ring offset of

@@ -39,9 +39,11 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   static_assert(YFIRST || !LATE, "the late ring request needs the full barrier of the y-first order");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);
-  double* RMy = ring + NS * SLOT;      // y minus values, item-indexed [v][item]
-  double* Fy = RMy + NF * NYI;         // y face fluxes: item's upper face
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + NF * NYI);
+  constexpr bool YT = C::YT;           // y items in thread order (scheme B), see below
+  constexpr int NYX = C::NYX;          // doubles per field of a y exchange array
+  double* RMy = ring + NS * SLOT;      // y minus values [v][slot of the item]
+  double* Fy = RMy + NF * NYX;         // y face fluxes: item's upper face
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(Fy + NF * NYX);
   double* red = reinterpret_cast<double*>(bars + NS);
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -51,14 +53,41 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   const bool mine = tx >= 1 && tx <= cols && ty < rows;          // thread tx owns cell ix = tx - 1
   // y items: cells (y_ix, y_c - 1), y_c = 0..TY+1; the last four threads repeat item NYI-1 (nothing stored)
   const int yit = min(tid, NYI - 1), y_c = yit / TX, y_ix = yit - y_c * TX;
-  const bool ystore = tid < NYI;
   const double gamma = g.gamma, gm1 = gamma - 1.0, inv_gm1 = 1.0 / gm1;
   const double dt = step_dt(sc, a.cur, a.cfl, a.dt_fixed);
   const double idx = g.inv_d[0], idy = g.inv_d[1], idz = g.inv_d[2];
   const int zb = k0 - R - 1;                                     // first plane loaded; ring slot of plane z = (z - zb) % NS
   const int cx = g.off[0] + i0 - G, cy = g.off[1] + j0 - G;      // cx = i0: even, so 16-byte aligned
   const int cellz = (ty + G) * BX + (tx - 1 + G);                // own column (also the x item of this thread)
-  const int celly = (y_c - 1 + G) * BX + (y_ix + G);
+  // Scheme A: the 252 items in linear order, item = cell (y_ix, y_c - 1); exchange slot = item index.  A half-warp
+  // then straddles ring rows (pitch 20): two-way bank conflicts on part of the y reads (with pitch 20
+  // no conflict-free placement exists next to 2 CTAs/SM).
+  // Scheme B (YT): items in THREAD ORDER.  Lane tx = 1..14 of row ty takes its own cell (tx-1, ty): a half-warp reads
+  // 14 consecutive doubles of one ring row.  The 28 items of rows -1 and TY go to the lanes tx = 0 / 15, each to
+  // the half-warp whose two spare banks (ring pitch 18: banks 2ty+5 and 2ty+4 mod 16, counted in doubles) are exactly
+  // the banks of that item: lane 0 takes (row -1, col 2ty+1) for ty <= 6, (row TY, col 13) for ty = 7, (row TY, col
+  // 2ty-17) for ty = 9..14; lane 15 takes (row -1, col 2ty), (row TY, col 12), (row TY, col 2ty-18).  Stencil, field
+  // and slot offsets shift every lane's bank alike, so all y ring reads are conflict-free.  The four lanes left over
+  // (ty = 8, 15) repeat their neighbour's cell (same address: a broadcast).  The exchange arrays mirror the ring's
+  // geometry — slot of item (col, row) = (row + 1) * BX + col + 1 — so the same bank matching holds there: a
+  // half-warp reads the 14 slots of the row above plus, for its two row -1 items, two slots of row 0 that fall on
+  // its spare banks.
+  int e_row = 0, e_col = 0;
+  bool e_item = false;
+  if (YT && (tx == 0 || tx == 15)) {
+    const int odd = (tx == 0) ? 1 : 0;
+    if (ty <= 6)                  { e_item = true; e_row = -1; e_col = 2 * ty + odd; }
+    else if (ty == 7)             { e_item = true; e_row = TY; e_col = 12 + odd; }
+    else if (ty >= 9 && ty <= 14) { e_item = true; e_row = TY; e_col = 2 * ty - 18 + odd; }
+    else                          { e_row = ty; e_col = (tx == 0) ? 0 : TX - 1; }
+  }
+  const bool xl = YT && (tx == 0 || tx == 15);
+  const int celly = !YT ? (y_c - 1 + G) * BX + (y_ix + G) : xl ? (e_row + G) * BX + (e_col + G) : cellz;
+  const int ys_own = !YT ? tid : (ty + 1) * BX + tx;                         // where every lane stores (edge slots: unused)
+  const int ys_x = (e_row + 1) * BX + e_col + 1;                             // slot of an extra item
+  const int ys_up = !YT ? min(tid + TX, NYI - 1) : (xl && e_item && e_row < 0) ? ys_x + BX : ys_own + BX;   // item above
+  const bool ystore = YT || tid < NYI;
+  const bool xstore_rm = YT && e_item && e_row == TY, xstore_fy = YT && e_item && e_row == -1;
 
   // red[62], red[63] (unused by the final reduction) hold the two split-phase barriers of the plane loop
   const uint32_t barY = smem_u32(&red[62]), barF = smem_u32(&red[63]);
@@ -187,7 +216,11 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
       recon_item<S, NF>(ring, o, plY, mi);
       if (ystore) {
 #pragma unroll
-        for (int v = 0; v < NF; ++v) RMy[v * NYI + tid] = mi[v];
+        for (int v = 0; v < NF; ++v) RMy[v * NYX + ys_own] = mi[v];
+      }
+      if (xstore_rm) {                                 // a second store: the extra lanes' items of row TY
+#pragma unroll
+        for (int v = 0; v < NF; ++v) RMy[v * NYX + ys_x] = mi[v];
       }
     }
     // barrier 1 (RMy written -> read).  YFIRST: a full barrier, the y fluxes follow at once.  Otherwise split-phase:
@@ -217,13 +250,16 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     // ---- y fluxes: face above item (between item and item + TX); the top row's result is not used
     auto yflux = [&]() {
       double mr[NF], F[NF];
-      const int up = min(tid + TX, NYI - 1);
 #pragma unroll
-      for (int v = 0; v < NF; ++v) mr[v] = RMy[v * NYI + up];
+      for (int v = 0; v < NF; ++v) mr[v] = RMy[v * NYX + ys_up];
       face_flux<S, 1, NF>(plY, mr, gamma, inv_gm1, F);
       if (ystore) {
 #pragma unroll
-        for (int v = 0; v < NF; ++v) Fy[v * NYI + tid] = F[v];
+        for (int v = 0; v < NF; ++v) Fy[v * NYX + ys_own] = F[v];
+      }
+      if (xstore_fy) {                                 // a second store: the extra lanes' faces below row 0
+#pragma unroll
+        for (int v = 0; v < NF; ++v) Fy[v * NYX + ys_x] = F[v];
       }
     };
     // barrier 2 (Fy written -> read) is split-phase in both orders
@@ -249,10 +285,11 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
     // ---- a5 + a6 (+ a7): finish the divergence, RK combination, store
     if (mine) {
       double out[NF];
-      const int yi = ty * TX + (tx - 1);               // item of cell (tx-1, ty-1): its upper face is our lower face
+      // slot of the item of cell (tx-1, ty-1): its upper face is our lower face; the next row's slot is our own item
+      const int yi = YT ? ty * BX + tx : ty * TX + (tx - 1), yj = YT ? yi + BX : yi + TX;
 #pragma unroll
       for (int v = 0; v < NF; ++v) {
-        const double L = fma(Fy[v * NYI + yi] - Fy[v * NYI + yi + TX], idy, Lacc[v]);
+        const double L = fma(Fy[v * NYX + yi] - Fy[v * NYX + yj], idy, Lacc[v]);
         if (MODE == MODE_STAGE1) out[v] = fma(dt, L, uc[v]);
         else out[v] = 0.5 * ua[v] + 0.5 * fma(dt, L, uc[v]);
         Uout[v * g.fstride + pc] = out[v];
