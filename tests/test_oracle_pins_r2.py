@@ -244,3 +244,96 @@ def test_wenoz_single_weight_probes_isolate_each_beta():
     be = wd.betas(*q)
     assert be[0] == pytest.approx(13 / 12 * (1.0 - 2.4 + 1.1) ** 2 + 0.25 * (1.0 - 4.8 + 3.3) ** 2, rel=1e-12)
     assert oracle.wenoz(*q) == pytest.approx(float(wd.wenoz(*q)), rel=1e-13)
+
+
+# --- round-2 mutation sweep (39 mutants of oracle/hard_oracle.cpp): three survived the suite; their pins:
+def _pressure_spike_data():
+    """rho smooth and well away from zero, PRESSURE with the spikes: WENO undershoots p, never rho"""
+    n = 20
+    i = np.arange(n)
+    var = (i >= 5) & (i <= 14)
+    p = np.ones(n)
+    p[7:13] = [0.01, 0.01, 4.98, 0.45, 0.03, 0.1]
+    rho = np.where(var, 1.0 + 0.3 * np.cos(0.9 * i), 1.0)
+    u = np.where(var, 0.03 + 0.02 * np.sin(1.3 * i), 0.03)       # slow: subsonic even where p = 0.01
+    v = np.where(var, 0.1 * np.cos(0.7 * i), 0.0)
+    w = np.where(var, -0.2 * np.sin(0.4 * i + 1.0), 0.0)
+    return rho, u, v, w, p
+
+
+def _pm(q):
+    pl = wd.wenoz(np.roll(q, 2), np.roll(q, 1), q, np.roll(q, -1), np.roll(q, -2))
+    mi = wd.wenoz(np.roll(q, -2), np.roll(q, -1), q, np.roll(q, 1), np.roll(q, 2))
+    return pl, mi
+
+
+def test_fallback_is_triggered_by_the_pressure_alone():
+    """G4: 'a reconstructed rho OR p <= 0'.  (mutant: only rho tested)"""
+    rho, u, v, w, p = _pressure_spike_data()
+    n, dx = rho.size, 0.05
+    W = np.stack([rho, u, v, w, p])
+    PL, MI = zip(*[_pm(q) for q in W])
+    assert PL[0].min() > 0.5 and MI[0].min() > 0.5                 # rho never triggers
+    bad = (PL[4] <= 0) | (MI[4] <= 0)
+    assert list(np.nonzero(bad)[0]) == [7, 8, 11, 12]
+    o = oracle.Oracle(n, 1, 1, G, oracle.BC_PERIODIC, scheme=0, spacing=(dx, 1.0, 1.0))
+    o.set_state(*[_as3d(a, 0) for a in _cons(rho, [u, v, w], p)])
+    L = np.stack([a.ravel() for a in o.rhs()])
+    assert o.fallbacks() == 4
+    rho0, u0, p0 = 1.0, 0.03, 1.0
+    E0 = p0 / (G - 1) + 0.5 * rho0 * u0 * u0
+    F0 = np.array([rho0 * u0, rho0 * u0 * u0 + p0, 0.0, 0.0, (E0 + p0) * u0])
+    face = lambda i: F0 - dx * L[:, :i + 1].sum(axis=1)
+    for i in (7, 11):                                              # between two fallen-back cells: cell averages
+        exp = _hll_textbook(W[:, i], W[:, i + 1])
+        assert np.abs(face(i) - exp).max() <= 1e-12 * np.abs(exp).max(), i
+
+
+def test_fallback_takes_the_radiation_energy_along():
+    """G19: E_rad 'follows the positivity fallback but does not trigger it'.  Between two fallen-back cells the
+    Rusanov flux is that of the two CELL values of E_rad (typed out); and E_rad <= 0 reconstructions alone trigger
+    nothing.  (mutant: E_rad keeps its WENO values in a fallen-back cell)"""
+    rho, u, v, w, p = _fallback_data()
+    n, dx = rho.size, 0.05
+    i = np.arange(n)
+    er = np.where((i >= 5) & (i <= 14), 2.0 + np.sin(1.1 * i), 2.0)
+    o = oracle.Oracle(n, 1, 1, G, oracle.BC_PERIODIC, scheme=0, spacing=(dx, 1.0, 1.0), radiation=True)
+    o.set_state(*[_as3d(a, 0) for a in _cons(rho, [u, v, w], p)])
+    o.set_rad_energy(_as3d(er, 0))
+    L5 = o.rhs(nf=6)[5].ravel()
+    assert o.fallbacks() == 4
+    face = lambda k: 2.0 * 0.3 - dx * L5[:k + 1].sum()             # face -1/2 lies in the uniform run: F = E u
+    for k in (7, 11):
+        cL, cR = np.sqrt(G * p[k] / rho[k]), np.sqrt(G * p[k + 1] / rho[k + 1])
+        alpha = max(abs(u[k]) + cL, abs(u[k + 1]) + cR)
+        exp = 0.5 * (er[k] * u[k] + er[k + 1] * u[k + 1]) - 0.5 * alpha * (er[k + 1] - er[k])
+        assert abs(face(k) - exp) <= 1e-12 * abs(exp), k
+    # spikes in E_rad alone (hydro smooth): WENO undershoots E_rad below zero, and nothing falls back
+    er2 = np.ones(n)
+    er2[7:13] = [0.01, 0.01, 4.98, 0.45, 0.03, 0.1]
+    pl, mi = _pm(er2)
+    assert min(pl.min(), mi.min()) < 0.0
+    o2 = oracle.Oracle(n, 1, 1, G, oracle.BC_PERIODIC, scheme=0, spacing=(dx, 1.0, 1.0), radiation=True)
+    o2.set_state(*[_as3d(a, 0) for a in _cons(np.ones(n), [0.3 + 0 * er2, 0 * er2, 0 * er2], np.ones(n))])
+    o2.set_rad_energy(_as3d(er2, 0))
+    o2.rhs(nf=6)
+    assert o2.fallbacks() == 0
+
+
+def test_next_dt_is_evaluated_after_the_source_update():
+    """G20: lambda (hence the next dt) belongs to the state the step RETURNS, i.e. after the source has changed the
+    pressure.  (mutant: max wavespeed taken before apply_source)"""
+    n = (12, 1, 1)
+    z = np.zeros(n[::-1])
+    gam, rho, cv = 5.0 / 3.0, 1.0, 1.5
+    o = oracle.Oracle(*n, gam, oracle.BC_PERIODIC, scheme=0, spacing=(0.1, 1.0, 1.0), radiation=True)
+    o.set_source(5.0, 3.0, 0.5, cv)                                 # kappa, c, a, cv: strong heating by the radiation
+    o.set_state(z + rho, z.copy(), z.copy(), z.copy(), z + 0.3)
+    o.set_rad_energy(z + 4.0)
+    dt0 = o.max_dt()
+    o.step_dt(0.05, 1)
+    E = o.get_state()[4].ravel()
+    assert E.min() > 0.5                                            # the gas has been heated a lot
+    p = (gam - 1.0) * E[0]                                          # gas at rest
+    assert abs(o.max_dt() - 0.1 / np.sqrt(gam * p / rho)) <= 1e-14 * o.max_dt()
+    assert o.max_dt() < 0.8 * dt0
