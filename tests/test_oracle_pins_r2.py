@@ -337,3 +337,28 @@ def test_next_dt_is_evaluated_after_the_source_update():
     p = (gam - 1.0) * E[0]                                          # gas at rest
     assert abs(o.max_dt() - 0.1 / np.sqrt(gam * p / rho)) <= 1e-14 * o.max_dt()
     assert o.max_dt() < 0.8 * dt0
+
+
+def test_negative_pressure_is_reported_as_non_physical():
+    """G4: 'a non-physical state is an error' — rho > 0 but p <= 0 (E below the kinetic energy).  (mutant: only rho)"""
+    z = np.zeros((1, 1, 8))
+    o = oracle.Oracle(8, 1, 1, G, oracle.BC_PERIODIC, scheme=1, spacing=(0.1, 1.0, 1.0))
+    E = z + 2.5
+    E[0, 0, 3] = 0.4                                               # kinetic energy there is 0.5: p < 0
+    with pytest.raises(oracle.OracleError):
+        o.set_state(z + 1.0, z + 1.0, z.copy(), z.copy(), E)
+
+
+def test_set_state_zeroes_the_radiation_energy_and_set_spacing_reevaluates_lambda():
+    """API contract shared with include/hard.h: hard_set_state zeroes E_rad; hard_set_spacing re-evaluates lambda."""
+    z = np.zeros((1, 1, 8))
+    o = oracle.Oracle(8, 1, 1, G, oracle.BC_PERIODIC, scheme=0, spacing=(0.1, 1.0, 1.0), radiation=True)
+    st = [z + 1.0, z + 0.5, z.copy(), z.copy(), z + 2.5]
+    o.set_state(*st)
+    o.set_rad_energy(z + 7.0)
+    assert o.get_rad_energy().min() == 7.0
+    o.set_state(*st)
+    assert not o.get_rad_energy().any()
+    dt1 = o.max_dt()
+    o._chk(o.L.oracle_set_spacing(o.h, 0.05, 1.0, 1.0), "set_spacing")
+    assert abs(o.max_dt() - 0.5 * dt1) <= 1e-15 * dt1
