@@ -9,6 +9,8 @@
 //  * split-phase barriers on mbarriers (arrive after producing, wait before consuming) wherever independent work
 //    lies in between: scheme B around the x phase and the plane conversion, scheme A around the x phase;
 //  * own-cell loads for the RK combination pinned early (volatile asm) so a whole phase covers their latency.
+//  * scheme B: y items in thread order with the 28 items of rows -1 and TY placed on the lanes whose spare banks they
+//    fall on, exchange arrays with the ring's pitch: every shared-memory load is bank-conflict-free (see `celly`).
 // Included by hard_kernels.cuh inside namespace hard.
 #pragma once
 
