@@ -57,7 +57,7 @@ __device__ __forceinline__ void cons_to_prim(const double U[5], double gm1, doub
 // minus value is the same function on the mirrored stencil, so the smoothness indicators are shared
 // (beta0' = beta2, beta1' = beta1, beta2' = beta0).  Algebraically identical to the definition, but
 // arranged for the fp64 pipe:
-//  * everything in terms of the four differences d1..d4 (candidates minus c are 2-term forms);
+//  * everything in terms of the four differences d1..d4 and their differences s_k (which the betas need anyway);
 //  * beta scaled by 12/13 (beta' = s^2 + 3/13 t^2, eps' = 12/13 eps): tau/(beta+eps) is unchanged;
 //  * weights d_k (1 + tau/B_k) multiplied through by 10 B0 B1 B2: X_k = (B_k + tau) prod_{j!=k} B_j with the
 //    integer multipliers (1, 6, 3), which needs no division; one reciprocal per face normalises.
@@ -77,16 +77,17 @@ __device__ __forceinline__ void wenoz_incr(double a, double b, double c, double 
   // X_k = (B_k + tau) prod_{j != k} B_j = P + tau M_k with M_k = prod_{j != k} B_j, P = B0 B1 B2: 4 DMUL + 3 DFMA
   const double M0 = B1 * B2, M1 = B0 * B2, M2 = B0 * B1, P = B0 * M0;
   const double X0 = fma(tau, M0, P), X1 = fma(tau, M1, P), X2 = fma(tau, M2, P);
-  const double Y = 6.0 * X1, X0t = 3.0 * X0, X2t = 3.0 * X2;
-  const double sp = (X0 + Y) + X2t, sm = (X2 + Y) + X0t;             // 10 x (sum of the unnormalised weights)
-  // 6 (q_k - c) for the plus side and 6 (p_k - c) for the minus side
-  // (5 d2 - 2 d1 = 2 t0 - d2 and 2 d4 - 5 d3 = 2 t2 + d3: one DFMA each)
-  const double q0 = fma(2.0, t0, -d2), q1 = fma(2.0, d3, d2), q2 = fma(4.0, d3, -d4);
-  const double p0 = fma(2.0, t2, d3), p1 = -fma(2.0, d2, d3), p2 = fma(-4.0, d2, d1);
-  const double np = fma(X2t, q2, fma(Y, q1, X0 * q0));
-  const double nm = fma(X0t, p2, fma(Y, p1, X2 * p0));
-  wp = np * fast_rcp(sp);
-  wm = nm * fast_rcp(sm);
+  const double Y = 6.0 * X1;
+  const double sp = fma(3.0, X2, X0 + Y), sm = fma(3.0, X0, X2 + Y);  // 10 x (sum of the unnormalised weights)
+  // 6 (q_k - c), 6 (p_k - c): the candidates' increments.  Relative to the MIDDLE candidate they are second differences
+  // the betas already hold: q0 - q1 = 2 (s0 - s1), q2 - q1 = s1 - s2, p0 - p1 = -2 (s1 - s2), p2 - p1 = -(s0 - s1), so
+  //   6 (plus  - c) = q1 + (2 X0 e0 + 3 X2 e2) / sp,    e0 = s0 - s1, e2 = s1 - s2,
+  //   6 (minus - c) = p1 - (3 X0 e0 + 2 X2 e2) / sm:   two products serve both faces.
+  const double q1 = fma(2.0, d3, d2), p1 = -fma(2.0, d2, d3);
+  const double A0 = X0 * (s0 - s1), A2 = X2 * (s1 - s2);
+  const double np = fma(3.0, A2, A0 + A0), nm = fma(3.0, A0, A2 + A2);
+  wp = fma(np, fast_rcp(sp), q1);
+  wm = fma(-nm, fast_rcp(sm), p1);
 }
 
 // a3, scheme B: MUSCL with the minmod limiter.  Branch-free: the slope is the argument of smaller
