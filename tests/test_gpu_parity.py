@@ -45,6 +45,48 @@ def test_one_step_random_state(scheme, variant, n, bc):
 
 
 @pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("bc", [wl.BC_PERIODIC, wl.BC_OUTFLOW])
+def test_supersonic_random_state(scheme, bc):
+    """Mach 0..2.5 in every direction and both senses (smooth modes + noise): the clamped (one-sided) branches of HLL / HLLC — SL >= 0 and
+    SR <= 0 — on most faces, subsonic ones in between."""
+    n = (37, 21, 19)
+    z, y, x = np.meshgrid((np.arange(n[2]) + 0.5) / n[2], (np.arange(n[1]) + 0.5) / n[1], (np.arange(n[0]) + 0.5) / n[0],
+                          indexing="ij")
+    rng = np.random.default_rng(314)
+    rho = 1.0 + 0.2 * np.sin(2 * np.pi * (x - z)) + 0.05 * (rng.random(x.shape) - 0.5)
+    prs = 1.0 + 0.2 * np.cos(2 * np.pi * (y + z)) + 0.05 * (rng.random(x.shape) - 0.5)
+    vel = [3.0 * np.sin(2 * np.pi * (x + y)), 3.0 * np.cos(2 * np.pi * (y - z)), 3.0 * np.sin(2 * np.pi * (z + x) + 1.0)]
+    E = prs / 0.4 + 0.5 * rho * (vel[0] ** 2 + vel[1] ** 2 + vel[2] ** 2)
+    w = wl.Workload("supersonic", n, 1.4, bc, (0.1, 0.07, 0.13), 0.4, nsteps=5,
+                    state=[rho, rho * vel[0], rho * vel[1], rho * vel[2], E])
+    _check(w, scheme, hard.VARIANT_FUSED, 1, TOL_1)
+    _check(w, scheme, hard.VARIANT_FUSED, 5, TOL_100)
+
+
+def test_positivity_fallback_is_taken_in_3d_and_matches():
+    """Scheme A on a field with density and pressure spikes in all three directions: the oracle reports fallbacks
+    (G4), the kernel's branch-free version of it gives the same step."""
+    import oracle
+    n = (30, 20, 18)
+    rng = np.random.default_rng(9)
+    shp = n[::-1]
+    rho = np.where(rng.random(shp) < 0.08, 0.01, 1.0) * (1.0 + 0.2 * rng.random(shp))
+    rho = np.where(rng.random(shp) < 0.04, 5.0, rho)
+    prs = np.where(rng.random(shp) < 0.08, 0.02, 1.0) * (1.0 + 0.2 * rng.random(shp))
+    vel = [0.4 * (rng.random(shp) - 0.5) for _ in range(3)]
+    E = prs / 0.4 + 0.5 * rho * (vel[0] ** 2 + vel[1] ** 2 + vel[2] ** 2)
+    st = [rho, rho * vel[0], rho * vel[1], rho * vel[2], E]
+    o = oracle.Oracle(*n, 1.4, wl.BC_PERIODIC, scheme=hard.SCHEME_WENO5Z_HLL, spacing=(0.1, 0.07, 0.13))
+    o.set_state(*st)
+    o.rhs()
+    assert o.fallbacks() > 200, o.fallbacks()
+    o.close()
+    w = wl.Workload("spikes", n, 1.4, wl.BC_PERIODIC, (0.1, 0.07, 0.13), 0.2, nsteps=1, state=st)
+    _check(w, hard.SCHEME_WENO5Z_HLL, hard.VARIANT_FUSED, 1, TOL_1)
+    _check(w, hard.SCHEME_WENO5Z_HLL, hard.VARIANT_PERDIR, 1, TOL_1)
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_sod_c0(scheme, variant):
     w = wl.sod(1000)
