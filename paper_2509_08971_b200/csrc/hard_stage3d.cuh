@@ -74,6 +74,7 @@ stage3d_kernel(const __grid_constant__ CUtensorMap tmap, const double* __restric
   // geometry — slot of item (col, row) = (row + 1) * BX + col + 1 — so the same bank matching holds there: a
   // half-warp reads the 14 slots of the row above plus, for its two row -1 items, two slots of row 0 that fall on
   // its spare banks.
+  static_assert(!YT || (BX == 18 && TX == 14 && TY == 16 && G == 2), "the bank matching of the extra y items is worked out for ring pitch 18");
   int e_row = 0, e_col = 0;
   bool e_item = false;
   if (YT && (tx == 0 || tx == 15)) {
