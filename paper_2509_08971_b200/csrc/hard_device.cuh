@@ -77,15 +77,17 @@ __device__ __forceinline__ void wenoz_incr(double a, double b, double c, double 
   // X_k = (B_k + tau) prod_{j != k} B_j = P + tau M_k with M_k = prod_{j != k} B_j, P = B0 B1 B2: 4 DMUL + 3 DFMA
   const double M0 = B1 * B2, M1 = B0 * B2, M2 = B0 * B1, P = B0 * M0;
   const double X0 = fma(tau, M0, P), X1 = fma(tau, M1, P), X2 = fma(tau, M2, P);
-  const double Y = 6.0 * X1;
-  const double sp = fma(3.0, X2, X0 + Y), sm = fma(3.0, X0, X2 + Y);  // 10 x (sum of the unnormalised weights)
   // 6 (q_k - c), 6 (p_k - c): the candidates' increments.  Relative to the MIDDLE candidate they are second differences
-  // the betas already hold: q0 - q1 = 2 (s0 - s1), q2 - q1 = s1 - s2, p0 - p1 = -2 (s1 - s2), p2 - p1 = -(s0 - s1), so
-  //   6 (plus  - c) = q1 + (2 X0 e0 + 3 X2 e2) / sp,    e0 = s0 - s1, e2 = s1 - s2,
-  //   6 (minus - c) = p1 - (3 X0 e0 + 2 X2 e2) / sm:   two products serve both faces.
+  // the betas already hold: q0 - q1 = 2 (s0 - s1), q2 - q1 = s1 - s2, p0 - p1 = -2 (s1 - s2), p2 - p1 = -(s0 - s1), so with
+  // the weights (X0, 6 X1, 3 X2) of the plus face and (3 X0, 6 X1, X2) of the minus face, e0 = s0 - s1, e2 = s1 - s2:
+  //   6 (plus  - c) = q1 + (2 X0 e0 + 3 X2 e2) / (X0 + 6 X1 + 3 X2),
+  //   6 (minus - c) = p1 - (3 X0 e0 + 2 X2 e2) / (3 X0 + 6 X1 + X2).
+  // Numerators and denominators are taken divided by 3 (the quotients do not change): one DFMA for each numerator on
+  // the two shared products, two for each denominator.
   const double q1 = fma(2.0, d3, d2), p1 = -fma(2.0, d2, d3);
   const double A0 = X0 * (s0 - s1), A2 = X2 * (s1 - s2);
-  const double np = fma(3.0, A2, A0 + A0), nm = fma(3.0, A0, A2 + A2);
+  const double np = fma(2.0 / 3.0, A0, A2), nm = fma(2.0 / 3.0, A2, A0);
+  const double sp = fma(1.0 / 3.0, X0, fma(2.0, X1, X2)), sm = fma(1.0 / 3.0, X2, fma(2.0, X1, X0));
   wp = fma(np, fast_rcp(sp), q1);
   wm = fma(-nm, fast_rcp(sm), p1);
 }
