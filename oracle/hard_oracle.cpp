@@ -34,8 +34,10 @@
 // restatement of a full step, and (tests/test_oracle_pins_r2.py, each failing under the matching mutation
 // of this file): wenoz against WENO5-Z rebuilt from its integral definition with numpy.polynomial;
 // outflow ghosts against the scalar upwind scheme that uniform-(u,p) flow reduces to; the G4 fallback
-// against textbook HLL fluxes of cell averages read off L(U) by telescoping.  No function here is
-// "parity unpinned".
+// against textbook HLL fluxes of cell averages read off L(U) by telescoping; and
+// (tests/test_oracle_eps_pin.py, round 3) the WENO-Z eps through the closed-form value eps/(18 s) on a one-cell spike,
+// degree-1 homogeneity down to data of 1e-12 and the linear-weight limit below eps.  No function here is
+// "parity unpinned" under the mutation sweeps run so far (DESIGN.md sections 2-3).
 
 #include <algorithm>
 #include <cmath>

@@ -74,10 +74,11 @@ def candidates(a, b, c, d, e):
     return [Q[k, 0] * v[k] + Q[k, 1] * v[k + 1] + Q[k, 2] * v[k + 2] for k in range(3)]
 
 
-def wenoz(a, b, c, d, e):
-    """Face value at i+1/2 from cell averages q[i-2..i+2]; scalars or numpy arrays."""
+def wenoz(a, b, c, d, e, eps=EPS):
+    """Face value at i+1/2 from cell averages q[i-2..i+2]; scalars or numpy arrays.  eps is a parameter so that
+    tests can show which values of it the data can tell apart (tests/test_oracle_eps_pin.py)."""
     be = betas(a, b, c, d, e)
     q = candidates(a, b, c, d, e)
     tau = np.abs(be[0] - be[2])
-    al = [D[k] * (1.0 + tau / (be[k] + EPS)) for k in range(3)]
+    al = [D[k] * (1.0 + tau / (be[k] + eps)) for k in range(3)]
     return (al[0] * q[0] + al[1] * q[1] + al[2] * q[2]) / (al[0] + al[1] + al[2])
