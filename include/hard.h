@@ -158,6 +158,37 @@ long long hard_launch_count(const hard_ctx*);
  * the roofline of the dominant kernel. */
 int hard_stage_time(hard_ctx*, int reset, double* ms, long long* launches);
 
+/* ---- one entry point for callers that must not allocate device memory -------------------------------------
+ * Everything above needs a workspace that somebody allocates: the library with cudaMalloc, or the caller before
+ * hard_bind_workspace.  A caller that can do neither when it needs the time step — a plugin running inside another
+ * framework's step that may only read the tensors it is handed, a process whose device pool was sized at start-up
+ * and whose policy forbids cudaMalloc afterwards, a diagnostic hook fired while the application owns all free HBM —
+ * uses this call instead.  It is the CFL reduction of row a7 (G6) on five caller-held fields:
+ *   *dt_out = 1 / max over cells and active directions of (|u_d| + c_s) / Delta_d,
+ * bit-equal to hard_set_state + hard_max_dt on the same fields and spacing (same operation order), and NaN if any
+ * cell is non-physical (non-finite, rho <= 0 or p <= 0).  A direction with n = 1 is inactive, as in hard_create.
+ *
+ * Pointers: rho, mx, my, mz, E and dt_out are DEVICE pointers on the current CUDA device (layout at the top of this
+ * file; dt_out addresses one double); the caller owns them.  The call only enqueues a 256-byte memset and one
+ * kernel on cuda_stream (NULL = default stream) and returns; read *dt_out after synchronising that stream.
+ * It calls no cudaMalloc, cudaFree or allocating library routine.  Its scratch (one partial maximum per 8192 cells,
+ * a ticket counter, a flag: 33 024 bytes) is a static __device__ array inside the library, resident on every GPU
+ * that loads the library until the process exits.  Hence the size limit: nx*ny*nz <= HARD_NOALLOC_MAX_CELLS
+ * (2^25 = 33 554 432 cells, e.g. 322^3; every 1-D config and the 128^3 Sedov mesh fit); larger meshes are rejected
+ * with HARD_ERR_ARG and a message naming the limit.
+ * First call on a device: it looks up the device address of that array (cudaGetSymbolAddress, once per device, with
+ * that device current); make this first call outside any stream capture.
+ * Sharing: all calls on a device use the same array.  The call clears the counter and the flag before each launch,
+ * so back-to-back calls on one stream are independent; calls whose kernels can overlap on the GPU (unordered
+ * streams, several host threads) race on the array and must be ordered by the caller.
+ * Errors: HARD_OK, HARD_ERR_ARG (bad size / null / host pointer / over the limit) or HARD_ERR_CUDA; text from
+ * hard_noalloc_last_error() (thread-local, valid until this thread's next hard_max_dt_noalloc). */
+#define HARD_NOALLOC_MAX_CELLS (1LL << 25)
+int hard_max_dt_noalloc(int nx, int ny, int nz, double gamma, double dx, double dy, double dz, const double* rho,
+                        const double* mx, const double* my, const double* mz, const double* E, double* dt_out,
+                        void* cuda_stream);
+const char* hard_noalloc_last_error(void);
+
 /* ---- environment variables read by the library (tuning / debugging; none is needed for normal use) -------
  *   HARD_LZ=<n>            planes per z-chunk of the fused stage kernel (default: a cost model, choose_Lz)
  *   HARD_NO_GRAPH=1        never replay CUDA graphs in hard_step* (launch-bound 1-D meshes then cost more per step)

@@ -11,8 +11,8 @@ INC = os.path.join(_HERE, "..", "include")
 LIB = os.path.join(_HERE, "libhard_b200.so")
 PROBE_LIB = os.path.join(_HERE, "libhard_probe.so")
 TARGETS = {
-    LIB: (["hard_api.cu"], ["hard_api.cu", "hard_kernels.cuh", "hard_stage3d.cuh", "hard_device.cuh",
-                            os.path.join(INC, "hard.h")]),
+    LIB: (["hard_api.cu", "hard_noalloc.cu"], ["hard_api.cu", "hard_noalloc.cu", "hard_kernels.cuh", "hard_stage3d.cuh",
+                                               "hard_device.cuh", os.path.join(INC, "hard.h")]),
     PROBE_LIB: (["hard_probe.cu"], ["hard_probe.cu", os.path.join(INC, "hard_probe.h")]),
 }
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

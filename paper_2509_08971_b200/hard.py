@@ -25,7 +25,8 @@ EXPORTS = ["hard_create", "hard_set_state", "hard_step", "hard_get_state", "hard
            "hard_bind_workspace", "hard_step_dt", "hard_get_time", "hard_last_error", "hard_launch_count",
            "hard_stage_time", "hard_enable_radiation", "hard_set_rad_energy",
            "hard_get_rad_energy", "hard_set_source", "hard_set_slab", "hard_halo_doubles", "hard_halo_pack",
-           "hard_halo_unpack", "hard_substep", "hard_lambda_ptr"]
+           "hard_halo_unpack", "hard_substep", "hard_lambda_ptr", "hard_max_dt_noalloc", "hard_noalloc_last_error"]
+NOALLOC_MAX_CELLS = 1 << 25          # HARD_NOALLOC_MAX_CELLS of include/hard.h
 
 _lib = None
 
@@ -76,6 +77,9 @@ def lib():
     L.hard_halo_unpack.argtypes = [vp, c_int, c_int, dp]
     L.hard_substep.argtypes = [vp, c_dbl, c_dbl, c_int]
     L.hard_lambda_ptr.argtypes = [vp, c_int, ctypes.POINTER(ctypes.c_void_p)]
+    L.hard_max_dt_noalloc.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_dbl] + [dp] * 6 + [vp]
+    L.hard_noalloc_last_error.restype = ctypes.c_char_p
+    L.hard_noalloc_last_error.argtypes = []
     _lib = L
     return L
 
@@ -112,6 +116,29 @@ def _ptr(a):
         return a.ctypes.data
     assert a.dtype.is_floating_point and a.element_size() == 8 and a.is_contiguous()
     return a.data_ptr()
+
+
+def max_dt_noalloc(rho, mx, my, mz, E, gamma, spacing, out, stream=None):
+    """hard_max_dt_noalloc: 1 / lambda_max of five device fields of shape (nz, ny, nx) into the one-element device
+    tensor `out`, without any device allocation (the reduction's scratch is a static array inside the library).
+
+    For callers that may not allocate on the GPU when they need dt (code running inside another framework's step,
+    fixed memory pools, hooks fired when no HBM is free) — see include/hard.h for the limit (NOALLOC_MAX_CELLS
+    cells), the first-call set-up and the rule that overlapping calls race.  Marshalling only: this function creates
+    no tensor; the call is asynchronous on `stream` (default: torch's current stream), so synchronise before reading
+    `out`, which holds NaN if the state is non-physical."""
+    L = lib()
+    nz, ny, nx = rho.shape
+    for a in (rho, mx, my, mz, E):
+        assert tuple(a.shape) == (nz, ny, nx) and a.is_cuda
+    assert out.is_cuda and out.numel() >= 1
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = L.hard_max_dt_noalloc(nx, ny, nz, float(gamma), *map(float, spacing), *[_ptr(a) for a in (rho, mx, my, mz, E)],
+                               _ptr(out), stream)
+    if rc != OK:
+        raise HardError(rc, L.hard_noalloc_last_error().decode())
 
 
 class Hard:
