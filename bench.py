@@ -29,15 +29,24 @@ if ROOT not in sys.path:
 METRIC = "fp64 cell-updates/sec per RK stage"
 UNIT = "cell-stage-updates/s"
 ALG_BYTES_PER_CELL_STAGE = 100.0     # stage 1 = 40 R + 40 W, stage 2 = 80 R + 40 W  => 100 B average
-# hand count of the method's minimal fp64 operations per cell-stage (1 FMA = 2 flop)
-# (A: 1300, B: 540 fp64-pipe instructions; 2 flop-equivalents each, the DFMA peak's own unit).  This is the round-1
-# count and it is kept fixed as the unit of work: it is LOWER than SURVEY.md §8(d)'s table (1 700-1 900 / 520-650
-# instructions, i.e. 3 400-3 800 / 1 040-1 300 in this unit), hence the conservative choice, and ncu's executed
-# counts back it (profiles/README.md).  A kernel that needs fewer instructions than this for the same update
-# raises `frac` legitimately.
-ALG_FLOP_PER_CELL_STAGE = {"A": 2600.0, "B": 1080.0}
+# roofline.frac (round 3) follows COUNTERS, not a chosen unit of work: the fp64-pipe instructions the stage kernel
+# actually EXECUTED per launch (ncu sm__inst_executed_pipe_fp64.sum x 32 lanes, collected by the ncu child run of
+# this same bench; a count, never a time) x 2 flop / the live CUDA-event launch time / the live DFMA peak.
+# Units of work one can divide by instead, all per cell-stage, fp64-pipe thread instructions:
+#   935   scheme A, what the committed device functions need with no redundancy (halo items, idle lanes)
+#   1 104 / 1 152   scheme A, executed by stage 1 / stage 2 (ncu, round-2 kernels; the fallback below)
+#   1 300 round 1's hand count, the unit `frac` used in rounds 1-2 -> now reported as work_unit_frac only
+#   1 700 - 1 900   SURVEY.md section 8(d)'s estimate (+-30 %; too high: it would put the kernel above the peak)
+WORK_UNIT_FP64_PER_CELL_STAGE = {"A": 1300.0, "B": 540.0}
+MINIMAL_FP64_PER_CELL_STAGE = {"A": 935.0, "B": None}
+# executed counts of the committed kernels from profiles/ (average of the two stage launches), used only when ncu
+# cannot run inside bench.py (missing binary, closed counters); the line then says so in roofline.frac_source
+FALLBACK_EXECUTED_FP64 = {"A": 1128.0, "B": 404.0}
 
 WORKLOADS = {"c4": (896, 10), "c3": (512, 20), "c2s": (256, 10)}
+# BASELINE.json configs[0..2]: launch-bound meshes ("run to t" configs; timed here over a fixed number of steps from
+# the initial state, CUDA-graph replay on, as Hard.run_to drives them).  name -> (generator, steps per --steps unit)
+LAUNCH_BOUND = {"c0": ("sod", 1000, 200), "c1": ("leblanc", 4096, 200), "c2": ("sedov", 128, 2)}
 
 
 def parse():
@@ -46,7 +55,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS) + sorted(LAUNCH_BOUND))
     ap.add_argument("--scheme", default="A", choices=["A", "B"])
     ap.add_argument("--variant", default="fused", choices=["fused", "perdir"])
     ap.add_argument("--radiation", action="store_true", help="NEXT-1: carry E_rad as a sixth advected field")
@@ -168,11 +177,16 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------ DRAM traffic (ncu child run)
-def ncu_stage_traffic(args, timeout=240):
-    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per stage-kernel launch, measured by running
-    this same bench (2 steps, nothing else) as a child under ncu and averaging the stage-1 and stage-2 launches of
-    the second step.  Only the byte counters come from the profiled run — never a time.  None if ncu is missing,
-    closed on the pool, or the child fails."""
+NCU_METRICS = ("dram__bytes_read.sum", "dram__bytes_write.sum", "sm__inst_executed_pipe_fp64.sum",
+               "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active", "smsp__inst_executed.sum",
+               "smsp__issue_active.avg.pct_of_peak_sustained_active")
+
+
+def ncu_stage_counters(args, timeout=300):
+    """Counters of the stage kernel per launch, measured by running this same bench (2 steps, nothing else) as a
+    child under ncu and averaging the stage-1 and stage-2 launches of the second step: DRAM bytes (roofline.traffic),
+    executed fp64-pipe and total warp instructions, fp64-pipe and issue utilisation.  Only counters come from the
+    profiled run — never a time.  (None, why) if ncu is missing, closed on the pool, or the child fails."""
     import shutil
     import signal
     import tempfile
@@ -180,7 +194,7 @@ def ncu_stage_traffic(args, timeout=240):
     if not os.path.exists(ncu):
         return None, "ncu not found"
     log = tempfile.NamedTemporaryFile(prefix="hard_ncu_", suffix=".csv", delete=False).name
-    cmd = [ncu, "--metrics", "dram__bytes_read.sum,dram__bytes_write.sum", "--clock-control", "none", "--print-units", "base",
+    cmd = [ncu, "--metrics", ",".join(NCU_METRICS), "--clock-control", "none", "--print-units", "base",
            "-k", "regex:stage", "-s", "2", "-c", "2", "--csv", "--log-file", log,
            sys.executable, os.path.abspath(__file__), "--workload", args.workload, "--scheme", args.scheme,
            "--variant", "fused", "--steps", "2", "--warmup", "0", "--no-e2e", "--no-cpu-baseline", "--no-variants",
@@ -201,11 +215,16 @@ def ncu_stage_traffic(args, timeout=240):
         per_launch = {}
         for r in rows[1:]:
             d = dict(zip(H, r))
-            per_launch.setdefault(d["ID"], 0.0)
-            per_launch[d["ID"]] += float(d["Metric Value"].replace(",", ""))
-        if len(per_launch) != 2:
-            return None, "ncu child run captured %d stage launches, expected 2" % len(per_launch)
-        return sum(per_launch.values()) / 2.0, "measured in this run: " + " ".join(cmd[:13]) + " ... (child bench, 2 steps)"
+            per_launch.setdefault(d["ID"], {})[d["Metric Name"]] = float(d["Metric Value"].replace(",", ""))
+        if len(per_launch) != 2 or any(set(NCU_METRICS) - set(m) for m in per_launch.values()):
+            return None, "ncu child run captured %d stage launches (expected 2) or lacks a metric" % len(per_launch)
+        avg = {k: sum(m[k] for m in per_launch.values()) / 2.0 for k in NCU_METRICS}
+        out = {"traffic": avg["dram__bytes_read.sum"] + avg["dram__bytes_write.sum"],
+               "fp64_warp_inst": avg["sm__inst_executed_pipe_fp64.sum"],
+               "fp64_pipe_busy_pct": avg["sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"],
+               "warp_inst": avg["smsp__inst_executed.sum"],
+               "issue_active_pct": avg["smsp__issue_active.avg.pct_of_peak_sustained_active"]}
+        return out, "measured in this run: " + " ".join(cmd[:2]) + " <6 counters> " + " ".join(cmd[3:13]) + " ... (child bench, 2 steps)"
     except Exception as ex:
         return None, "ncu child run: %s" % str(ex)[:160]
     finally:
@@ -213,6 +232,67 @@ def ncu_stage_traffic(args, timeout=240):
             os.unlink(log)
         except OSError:
             pass
+
+
+# ------------------------------------------------------------------------------------ launch-bound configs
+def launch_bound_measure(name, scheme, units, warm_units, local):
+    """C0 / C1 / C2 (BASELINE.json configs[0..2]): K = units * steps-per-unit Heun steps from the initial state on
+    torch's current (capturable) stream, so hard_step replays its two-step CUDA graph; device-timed with CUDA events.
+    The state is tiny (C0: 40 KB) and lives in L2: the figure is launch latency, not bandwidth — reported as such."""
+    import torch
+    from paper_2509_08971_b200 import hard
+    from paper_2509_08971_b200 import workloads as wl
+    gen, n, per = LAUNCH_BOUND[name]
+    w = getattr(wl, gen)(n)
+    k = max(units, 1) * per
+    h = hard.Hard(*w.n, w.gamma, w.bc, scheme=hard.SCHEME_WENO5Z_HLL if scheme == "A" else hard.SCHEME_MUSCL_HLLC, spacing=w.spacing)
+    st = [torch.from_numpy(__import__("numpy").ascontiguousarray(a)).cuda() for a in w.state]
+    h.set_state(*st)
+    h.step(w.cfl, max(warm_units, 1) * per)              # warm-up: graph capture + instantiation happen here
+    h.set_state(*st)
+    stream = torch.cuda.current_stream()
+    smp = ClockSampler(local)
+    smp.start()
+    time.sleep(0.3)
+    l0 = h.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.time()
+    e0.record(stream)
+    h.step(w.cfl, k)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    t_sim, steps_done = h.time()                         # surfaces a latched non-physical state
+    cells = w.n[0] * w.n[1] * w.n[2]
+    out = {"value": cells * 2.0 * k / (ms * 1e-3), "unit": UNIT, "workload": "%s %s" % (name, w.name), "cells": cells,
+           "steps": k, "us_per_step": ms * 1e3 / k, "ms_per_step": ms / k, "gpu_launches": h.launch_count() - l0,
+           "graph_replay": os.environ.get("HARD_NO_GRAPH") is None, "sim_time": t_sim, "steps_done": steps_done,
+           "clocks": smp.stop(t0, t1)}
+    h.close()
+    return out
+
+
+def run_launch_bound(args):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:                                      # a 1 000-cell mesh does not shard: rank 0 alone measures it
+        return
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the CUDA path has no CPU fallback", file=sys.stderr, flush=True)
+        raise SystemExit(3)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    m = launch_bound_measure(args.workload, args.scheme, args.steps, args.warmup, local)
+    line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": 1, "steps": m["steps"], "warmup": args.warmup * LAUNCH_BOUND[args.workload][2],
+            "ms_per_step": m["ms_per_step"], "us_per_step": m["us_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": m["workload"] + " (BASELINE.json configs[%s]); launch-bound: 4 launches per step, CUDA-graph replay of two steps" % args.workload[1],
+                       "scheme": args.scheme, "l2": "state fits in L2 by design of the config; the figure is launch latency"},
+            "roofline": None, "roofline_note": "launch-latency bound (DESIGN.md section 1): no bandwidth or ALU roofline applies",
+            "e2e": None, "cpu_baseline": None, "clocks": m["clocks"], "gpu_launches": m["gpu_launches"]}
+    print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------ CUDA arm
@@ -320,14 +400,29 @@ def run_cuda(args):
     else:
         cell_stages_per_launch = cells * 2.0 * K / max(stage_launches, 1)
     alg_gbs = cell_stages_per_launch * alg_bytes / (per_launch_ms * 1e-3) / 1e9
-    alg_tflops = cell_stages_per_launch * ALG_FLOP_PER_CELL_STAGE[args.scheme] / (per_launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": ("stage3d_kernel<%s, %d, stage 1|2>" % (args.scheme, nfields)) if variant == hard.VARIANT_FUSED else ("stage_kernel<%s, %d> per direction + axpy_kernel" % (args.scheme, nfields)), "achieved": alg_tflops, "peak": fp64_peak,
-                "unit": "TFLOP/s", "frac": alg_tflops / fp64_peak if fp64_peak else None,
+    def tflops(fp64_per_cell_stage):
+        return cell_stages_per_launch * 2.0 * fp64_per_cell_stage / (per_launch_ms * 1e-3) / 1e12
+
+    executed = FALLBACK_EXECUTED_FP64[args.scheme] * (6.0 / 5.0 if args.radiation else 1.0)
+    unit_tflops = tflops(WORK_UNIT_FP64_PER_CELL_STAGE[args.scheme])
+    roofline = {"bound": "alu", "kernel": ("stage3d_kernel<%s, %d, stage 1|2>" % (args.scheme, nfields)) if variant == hard.VARIANT_FUSED else ("stage_kernel<%s, %d> per direction + axpy_kernel" % (args.scheme, nfields)),
+                "achieved": tflops(executed), "peak": fp64_peak,
+                "unit": "TFLOP/s", "frac": tflops(executed) / fp64_peak if fp64_peak else None,
+                "frac_source": "executed fp64-pipe instructions per cell-stage from profiles/ (ncu did not run inside this bench)",
+                "executed_fp64_per_cell_stage": executed, "fp64_pipe_busy_pct": None, "issue_active_pct": None,
+                "warp_inst_per_cell_stage": None,
+                "work_unit_frac": unit_tflops / fp64_peak if fp64_peak else None,
+                "work_unit_fp64_per_cell_stage": WORK_UNIT_FP64_PER_CELL_STAGE[args.scheme],
+                "minimal_fp64_per_cell_stage": MINIMAL_FP64_PER_CELL_STAGE[args.scheme],
+                "useful_frac": (tflops(MINIMAL_FP64_PER_CELL_STAGE[args.scheme]) / fp64_peak)
+                               if (fp64_peak and MINIMAL_FP64_PER_CELL_STAGE[args.scheme] and not args.radiation) else None,
+                "units_note": "per cell-stage, fp64-pipe thread instructions (1 instruction = 2 flop, the DFMA peak's unit): "
+                              "frac uses what the kernel executed (ncu); work_unit_frac the fixed round-1 hand count "
+                              "(SURVEY 8(d) estimated 1700-1900 for A, too high); useful_frac the count with no redundancy",
                 "traffic": None, "traffic_note": "not measured in this run",
                 "alg_bytes_per_launch": slab_cells * alg_bytes,
                 "peak_source": "measured live: hard_probe_fp64_peak (DFMA chains on all SMs, libhard_probe.so)",
-                "avg_launch_ms": per_launch_ms, "launches_timed": stage_launches,
-                "alg_flop_per_cell_stage": ALG_FLOP_PER_CELL_STAGE[args.scheme]}
+                "avg_launch_ms": per_launch_ms, "launches_timed": stage_launches}
     roofline_hbm = {"bound": "hbm", "achieved": alg_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": alg_gbs / hbm_peak,
                     "frac_of_nominal_8TBs": alg_gbs / 8000.0, "peak_source": hbm_src,
                     "alg_bytes_per_cell_stage": alg_bytes}
@@ -375,37 +470,68 @@ def run_cuda(args):
     if rank == 0 and world == 1 and not args.no_variants and not args.radiation and variant == hard.VARIANT_FUSED:
         variants = {}
         other = "B" if args.scheme == "A" else "A"
-        for name, sch, var, k in (("perdir_" + args.scheme, args.scheme, hard.VARIANT_PERDIR, 3),
-                                  ("fused_" + other, other, hard.VARIANT_FUSED, max(3, K // 2))):
+        n3, _ = WORKLOADS["c3"]
+        # name, mesh, scheme, variant, steps, sixth field: every number BASELINE.md section 4 quotes has a twin here,
+        # each with its own clock record (sampled over its own timed region)
+        for name, nn, sch, var, k, rad in (("perdir_" + args.scheme, n, args.scheme, hard.VARIANT_PERDIR, 3, False),
+                                           ("fused_" + other, n, other, hard.VARIANT_FUSED, max(3, K // 2), False),
+                                           ("perdir_" + other, n, other, hard.VARIANT_PERDIR, 3, False),
+                                           ("fused_A6_c3", n3, "A", hard.VARIANT_FUSED, 5, True)):
             try:
-                wv = wl.turbulence(n, nsteps=k, device=dev)
+                wv = wl.turbulence(nn, nsteps=k, device=dev)
                 hv = hard.Hard(*wv.n, wv.gamma, wv.bc, scheme=hard.SCHEME_WENO5Z_HLL if sch == "A" else hard.SCHEME_MUSCL_HLLC,
-                               variant=var, spacing=wv.spacing)
-                hv.set_state(*wv.state)
+                               variant=var, spacing=wv.spacing, radiation=rad)
+                er = (1.0 + 0.3 * wv.state[0]) if rad else None
+
+                def load():
+                    hv.set_state(*wv.state)
+                    if rad:
+                        hv.set_rad_energy(er)
+                load()
                 hv.step(wv.cfl, 1)
-                hv.set_state(*wv.state)
+                load()
                 l0 = hv.launch_count()
+                smp = ClockSampler(local)
+                smp.start()
+                time.sleep(0.3)
                 ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 torch.cuda.synchronize()
+                tv0 = time.time()
                 ev0.record(stream)
                 hv.step(wv.cfl, k)
                 ev1.record(stream)
                 torch.cuda.synchronize()
+                tv1 = time.time()
                 msv = ev0.elapsed_time(ev1)
                 hv.time()                                  # surfaces a latched non-physical state
-                variants[name] = {"value": cells * 2.0 * k / (msv * 1e-3), "unit": UNIT, "steps": k, "warmup": 1,
+                nc = nn ** 3
+                variants[name] = {"value": nc * 2.0 * k / (msv * 1e-3), "unit": UNIT, "steps": k, "warmup": 1,
+                                  "workload": "%d^3" % nn, "fields": 6 if rad else 5,
                                   "ms_per_step": msv / k, "gpu_launches": hv.launch_count() - l0,
-                                  "alg_GBs": cells * 200.0 * k / (msv * 1e-3) / 1e9}
+                                  "alg_GBs": nc * (240.0 if rad else 200.0) * k / (msv * 1e-3) / 1e9,
+                                  "clocks": smp.stop(tv0, tv1)}
                 hv.close()
-                del hv, wv
+                del hv, wv, er
                 torch.cuda.empty_cache()
             except Exception as ex:
                 variants[name] = {"value": None, "error": str(ex)[:200]}
+        for lb in ("c0", "c1", "c2"):                      # BASELINE.json configs[0..2]: launch-bound, us per step
+            try:
+                variants[lb + "_" + args.scheme] = launch_bound_measure(lb, args.scheme, 5, 1, local)
+            except Exception as ex:
+                variants[lb + "_" + args.scheme] = {"value": None, "error": str(ex)[:200]}
 
     if rank == 0 and world == 1 and not args.no_ncu_traffic and variant == hard.VARIANT_FUSED and not shard:
-        traffic, note = ncu_stage_traffic(args)
-        roofline["traffic"] = traffic
+        ctr, note = ncu_stage_counters(args)
         roofline["traffic_note"] = note + "; average of one stage-1 and one stage-2 launch; algorithmic bytes per launch in alg_bytes_per_launch"
+        if ctr is not None:
+            roofline["traffic"] = ctr["traffic"]
+            executed = ctr["fp64_warp_inst"] * 32.0 / cells
+            roofline.update({"achieved": tflops(executed), "frac": tflops(executed) / fp64_peak if fp64_peak else None,
+                             "frac_source": "executed fp64-pipe instructions of this run's ncu child (sm__inst_executed_pipe_fp64.sum x 32 "
+                                            "lanes per launch) x 2 flop / live CUDA-event launch time / live DFMA peak",
+                             "executed_fp64_per_cell_stage": executed, "fp64_pipe_busy_pct": ctr["fp64_pipe_busy_pct"],
+                             "issue_active_pct": ctr["issue_active_pct"], "warp_inst_per_cell_stage": ctr["warp_inst"] * 32.0 / cells})
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -434,6 +560,8 @@ def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload in LAUNCH_BOUND:
+        run_launch_bound(args)
     else:
         run_cuda(args)
 

@@ -306,6 +306,7 @@ int perdir_residual(hard_ctx* c, const CUtensorMap& tm, const double* Usrc, doub
     if (e != cudaSuccess) return fail(c, HARD_ERR_NOMEM, std::string("cudaMalloc (per-direction residual): ") + cudaGetErrorString(e));
     c->Rres = (double*)r;
     c->rres_owned = true;
+    CK(cudaMemsetAsync(r, 0, state_bytes(c), c->stream));   // ghost layers of the residual are never written: defined from the start
   }
   int first = 1;
   for (int d = 0; d < 3; ++d) {
@@ -471,8 +472,15 @@ hard_ctx* hard_create(int nx, int ny, int nz, double gamma, int bc) {
     g_create_error = std::string("hard_create: no usable CUDA device (") + cudaGetErrorString(e) + "); there is no CPU fallback";
     return nullptr;
   }
-  if (prop.major < 10) {
-    g_create_error = "hard_create: kernels are built for sm_100a only";
+  // The library holds one cubin (sm_100a, no PTX): ask the runtime whether THIS device can run it instead of
+  // guessing from the compute capability (an sm_103 / sm_12x part would pass "major >= 10" and fail at the first launch).
+  cudaFuncAttributes fa;
+  if (prop.major != 10 || prop.minor != 0 || cudaFuncGetAttributes(&fa, cfl_kernel) != cudaSuccess) {
+    cudaGetLastError();
+    char buf[160];
+    snprintf(buf, sizeof buf, "hard_create: kernels are built for sm_100a only (device %d is sm_%d%d); there is no CPU fallback",
+             dev, prop.major, prop.minor);
+    g_create_error = buf;
     return nullptr;
   }
   hard_ctx* c = new hard_ctx();
@@ -652,7 +660,10 @@ int hard_bind_workspace(hard_ctx* c, void* dev, size_t bytes) {
   c->ws = dev;
   c->ws_bytes = bytes;
   c->ws_owned = false;
-  CK(cudaMemsetAsync(c->ws, 0, hard_workspace_bytes(c), c->stream));
+  // zero everything carve() may hand out: also the residual of the per-direction variant when the lent buffer is
+  // large enough for it although the fused variant is selected now
+  const size_t with_resid = 256 + 3 * align_up(state_bytes(c), 256);
+  CK(cudaMemsetAsync(c->ws, 0, bytes >= with_resid ? with_resid : hard_workspace_bytes(c), c->stream));
   carve(c);
   return HARD_OK;
 }
@@ -667,8 +678,7 @@ int hard_set_state(hard_ctx* c, const double* rho, const double* mx, const doubl
     if ((rc = copy_field(c, c->U + f * c->g.fstride, src[f], true))) return rc;
   if (c->nf == 6) CK(cudaMemsetAsync(c->U + 5 * c->g.fstride, 0, (size_t)c->g.fstride * sizeof(double), c->stream));
   CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
-  c->steps_enq = 0;
-  c->gen++;
+  c->steps_enq = 0;                                      // even: a captured two-step graph stays valid (it bakes in no state value)
   c->have_state = true;
   c->err.clear();
   if ((rc = launch_cfl(c, c->U, 0))) return rc;

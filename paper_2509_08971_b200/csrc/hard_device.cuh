@@ -153,6 +153,8 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     // k = rho (u_n - S) (neither U_K nor F_K is formed), the star flux F_K + S_K (U*_K - U_K) with
     // U*_K = (pbar D* - G) / (S_K - S*), D* = (0, 1, 0, 0, S*), is (1 - g) G + g pbar D*, g = S_K / (S_K - S*).
     // S clamped to zero on the supersonic side makes G = F_K and g = 0: no branch, no select on the result.
+    // h = 1 - g = -S* / (S_K - S*) is formed directly and g as 1 - h, so that a stationary contact (S* = +-0) gives
+    // h = 0 and g = 1 EXACTLY and the flux is (0, pbar, 0, 0, 0) to the last bit, as in the oracle's tie-break (G5).
     const bool left = Ss > 0.0;
     double W[5];
 #pragma unroll
@@ -163,7 +165,7 @@ __device__ __forceinline__ void riemann_flux(const double WL[5], const double WR
     const double d = W[1] - SKc, k = W[0] * d;
     const double v2 = fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3]));
     const double G4 = fma(0.5 * k, v2, W[4] * fma(d, inv_gm1, W[1]));
-    const double g = SKc * fast_rcp(SK - Ss), h = 1.0 - g, gp = g * pbar;
+    const double h = sub ? -Ss * fast_rcp(SK - Ss) : 1.0, g = 1.0 - h, gp = g * pbar;
     F[0] = h * k;
     F[1] = fma(h, fma(k, W[1], W[4]), gp);
     F[2] = h * (k * W[2]);

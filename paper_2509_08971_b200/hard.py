@@ -265,7 +265,8 @@ class Hard:
 
         Far from t_end the steps are enqueued in batches (one host synchronisation per batch instead of two per
         step; on launch-bound meshes the batch replays a CUDA graph): a batch covers at most a quarter of the
-        remaining time at the current dt, so it cannot reach t_end unless dt quadruples inside it — checked.
+        remaining time at the current dt and at most 256 steps, so it cannot reach t_end unless dt quadruples within
+        256 steps — checked (an overshoot raises; 256 keeps the graph-replay benefit, one sync per 256 steps).
         The dt sequence is the same as stepping one by one: dt_n = cfl / lambda(U^n) is evaluated on the device."""
         n = 0
         while n < max_steps:
@@ -277,7 +278,7 @@ class Hard:
                 self.step_dt(t_end - t, 1)
                 n += 1
                 break
-            batch = min(int(0.25 * (t_end - t) / dt), max_steps - n, 4096)
+            batch = min(int(0.25 * (t_end - t) / dt), max_steps - n, 256)
             if batch >= 8:
                 self.step(cfl, batch)
                 n += batch

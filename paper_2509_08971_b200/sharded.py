@@ -176,7 +176,12 @@ class ShardedHard:
     def __init__(self, n, gamma, bc, scheme=hard.SCHEME_WENO5Z_HLL, spacing=None, radiation=False, comm=None):
         if comm is None:                       # NCCL moves device buffers itself; gloo needs the host staging
             import torch.distributed as dist
-            comm = (DistComm if dist.get_backend() == "nccl" else HostStagedComm)(bc == hard.BC_PERIODIC)
+            # a group initialised without an explicit backend reports a composite string ("cuda:nccl,cpu:gloo")
+            use_nccl = "nccl" in str(dist.get_backend()).lower()
+            comm = (DistComm if use_nccl else HostStagedComm)(bc == hard.BC_PERIODIC)
+            if comm.rank == 0:
+                import sys
+                print("ShardedHard: %s (backend %s)" % (type(comm).__name__, dist.get_backend()), file=sys.stderr)
         self.comm = comm
         self.slab = Slab(n, gamma, bc, self.comm.rank, self.comm.world, scheme, spacing, radiation)
 

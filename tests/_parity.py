@@ -21,6 +21,17 @@ def field_errors(gpu, orc):
     return errs
 
 
+def pointwise_errors(gpu, orc):
+    """max over cells of |gpu - orc| / |orc| for the strictly positive fields rho and E (fields 0 and 4): the cell-by-cell
+    relative error, which the field norm above cannot see where a field spans many decades."""
+    out = []
+    for f in (0, 4):
+        a, b = gpu[f], orc[f]
+        assert np.all(b > 0)
+        out.append(float((np.abs(a - b) / b).max()))
+    return out
+
+
 def run_both(w, scheme, variant=hard.VARIANT_FUSED, nsteps=1, cfl=None, dt=None, state=None):
     """Returns (gpu_fields, oracle_fields, (gpu_dt0, orc_dt0), (gpu_t, orc_t))."""
     cfl = w.cfl if cfl is None else cfl
