@@ -404,7 +404,8 @@ def run_cuda(args):
         return cell_stages_per_launch * 2.0 * fp64_per_cell_stage / (per_launch_ms * 1e-3) / 1e12
 
     executed = FALLBACK_EXECUTED_FP64[args.scheme] * (6.0 / 5.0 if args.radiation else 1.0)
-    unit_tflops = tflops(WORK_UNIT_FP64_PER_CELL_STAGE[args.scheme])
+    work_unit = WORK_UNIT_FP64_PER_CELL_STAGE[args.scheme] * (6.0 / 5.0 if args.radiation else 1.0)
+    unit_tflops = tflops(work_unit)
     roofline = {"bound": "alu", "kernel": ("stage3d_kernel<%s, %d, stage 1|2>" % (args.scheme, nfields)) if variant == hard.VARIANT_FUSED else ("stage_kernel<%s, %d> per direction + axpy_kernel" % (args.scheme, nfields)),
                 "achieved": tflops(executed), "peak": fp64_peak,
                 "unit": "TFLOP/s", "frac": tflops(executed) / fp64_peak if fp64_peak else None,
@@ -412,7 +413,7 @@ def run_cuda(args):
                 "executed_fp64_per_cell_stage": executed, "fp64_pipe_busy_pct": None, "issue_active_pct": None,
                 "warp_inst_per_cell_stage": None,
                 "work_unit_frac": unit_tflops / fp64_peak if fp64_peak else None,
-                "work_unit_fp64_per_cell_stage": WORK_UNIT_FP64_PER_CELL_STAGE[args.scheme],
+                "work_unit_fp64_per_cell_stage": work_unit,
                 "minimal_fp64_per_cell_stage": MINIMAL_FP64_PER_CELL_STAGE[args.scheme],
                 "useful_frac": (tflops(MINIMAL_FP64_PER_CELL_STAGE[args.scheme]) / fp64_peak)
                                if (fp64_peak and MINIMAL_FP64_PER_CELL_STAGE[args.scheme] and not args.radiation) else None,
@@ -515,6 +516,40 @@ def run_cuda(args):
                 torch.cuda.empty_cache()
             except Exception as ex:
                 variants[name] = {"value": None, "error": str(ex)[:200]}
+        # NEXT-4 on the one GPU there is: the same mesh as two z-slabs of 448 planes emulated in this process
+        # (sharded.LocalGroup: the ranks' phases in lockstep, halos packed, copied device-to-device and unpacked, lambda
+        # max-reduced in place, exactly the sequence ShardedHard.step runs over NCCL).  Not a scaling number: it shows
+        # what the pack / unpack / reduction and the split stage launches cost per step next to the single domain.
+        try:
+            from paper_2509_08971_b200 import sharded
+            k = 3
+            wv = wl.turbulence(n, nsteps=k, device=dev)
+            grp = sharded.LocalGroup(wv.n, wv.gamma, wv.bc, 2, scheme=scheme, spacing=wv.spacing)
+            grp.set_state(wv.state)
+            grp.step(wv.cfl, 1)
+            grp.set_state(wv.state)
+            l0 = sum(sl.h.launch_count() for sl in grp.slabs)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            grp.step(wv.cfl, k)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            msv = ev0.elapsed_time(ev1)
+            for sl in grp.slabs:
+                sl.h.time()
+            variants["sharded_local_2x%d_%s" % (n // 2, args.scheme)] = {
+                "value": cells * 2.0 * k / (msv * 1e-3), "unit": UNIT, "steps": k, "warmup": 1, "workload": "%d^3 as 2 z-slabs on ONE GPU" % n,
+                "ms_per_step": msv / k, "overhead_ms_per_step_vs_single_domain": msv / k - ms / K,
+                "gpu_launches": sum(sl.h.launch_count() for sl in grp.slabs) - l0,
+                "halo_bytes_per_step": 2 * 2 * 2 * grp.slabs[0].h.halo_doubles() * 8,
+                "note": "LocalGroup emulation (no NCCL, one process); not a multi-GPU measurement"}
+            for sl in grp.slabs:
+                sl.close()
+            del grp, wv
+            torch.cuda.empty_cache()
+        except Exception as ex:
+            variants["sharded_local_2"] = {"value": None, "error": str(ex)[:200]}
         for lb in ("c0", "c1", "c2"):                      # BASELINE.json configs[0..2]: launch-bound, us per step
             try:
                 variants[lb + "_" + args.scheme] = launch_bound_measure(lb, args.scheme, 5, 1, local)
