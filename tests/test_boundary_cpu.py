@@ -137,3 +137,32 @@ def test_reference_arm_prints_contract_line():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "cell-stage-updates/s"
+
+
+def test_noalloc_entry_point_checks_arguments_before_touching_a_device():
+    """hard_max_dt_noalloc (include/hard.h): size and null checks come first and need no GPU; on a box without one a
+    well-formed call fails loudly with HARD_ERR_CUDA (no CPU fallback), it does not compute anything on the host."""
+    import ctypes
+    import torch
+    from paper_2509_08971_b200 import hard
+    L = hard.lib()
+    buf = (ctypes.c_double * 8)()
+    p = ctypes.addressof(buf)
+    err = lambda: L.hard_noalloc_last_error().decode()
+    assert L.hard_max_dt_noalloc(0, 1, 1, 1.4, 1.0, 1.0, 1.0, p, p, p, p, p, p, None) == hard.ERR_ARG
+    assert L.hard_max_dt_noalloc(8, 1, 1, 1.0, 1.0, 1.0, 1.0, p, p, p, p, p, p, None) == hard.ERR_ARG          # gamma <= 1
+    assert L.hard_max_dt_noalloc(8, 1, 1, 1.4, 0.0, 1.0, 1.0, p, p, p, p, p, p, None) == hard.ERR_ARG          # dx <= 0
+    assert L.hard_max_dt_noalloc(1, 1, 1, 1.4, 1.0, 1.0, 1.0, p, p, p, p, p, p, None) == hard.ERR_ARG          # no active direction
+    assert L.hard_max_dt_noalloc(8, 1, 1, 1.4, 1.0, 1.0, 1.0, p, p, None, p, p, p, None) == hard.ERR_ARG and "null" in err()
+    assert L.hard_max_dt_noalloc(4096, 4096, 3, 1.4, 1.0, 1.0, 1.0, p, p, p, p, p, p, None) == hard.ERR_ARG    # 50 331 648 cells
+    assert "HARD_NOALLOC_MAX_CELLS" in err() and str(hard.NOALLOC_MAX_CELLS) in err()
+    assert hard.NOALLOC_MAX_CELLS == 1 << 25
+    hdr = open(os.path.join(ROOT, "include", "hard.h")).read()
+    assert "#define HARD_NOALLOC_MAX_CELLS (1LL << 25)" in hdr
+    if not torch.cuda.is_available():
+        rc = L.hard_max_dt_noalloc(8, 1, 1, 1.4, 1.0, 1.0, 1.0, p, p, p, p, p, p, None)
+        assert rc == hard.ERR_CUDA and "no CPU fallback" in err()
+    # the static scratch is in the library image: a 33 024-byte object in its device code, no allocation call in the source
+    src = open(os.path.join(ROOT, "paper_2509_08971_b200", "csrc", "hard_noalloc.cu")).read()
+    code = re.sub(r"//.*", "", src)
+    assert "cudaMalloc" not in code and "cudaFree" not in code and "cudaGetSymbolAddress" in code
